@@ -1,0 +1,129 @@
+/*
+ * vx.h -- C ABI of the B200-native VaultxGPU plotting hot path (libvx.so).
+ *
+ * The library computes, for a plot (K, key):
+ *
+ *   Table 1  all 2^K records (n, H(n)), n in [0, 2^K), H(n) = first 8 bytes of the BLAKE3 keyed
+ *            hash of the NONCE_SIZE little-endian bytes of n (read big-endian), grouped into 2^24
+ *            buckets by the hash prefix  H >> 40       (PAPER.md L41-43 I-A, L81 III-A, L91 III-B)
+ *   Table 2  for every bucket, every pair of its records whose hashes differ by less than
+ *            T = 2^(64-K), as (n_first, n_second), first = smaller (H, n)
+ *                                                       (PAPER.md L65 II-B, L81 III-A)
+ *
+ * PAPER.md = /root/reference/PAPER.md (arxiv/paper_2606_14007).  Where the paper leaves the record
+ * layout, widths, bucket rule or predicate open, the readings are A1..A18 of SURVEY.md 8(c),
+ * restated in DESIGN.md.  Everything runs in hand-written CUDA kernels for sm_100a; there is no
+ * CPU fallback: without a CUDA device every compute call returns VX_ERR_CUDA.
+ *
+ * Conventions
+ *   - every call returns vx_status (no exceptions, no errno, no abort);
+ *   - `dev_*` pointers are DEVICE pointers owned by the caller (PyTorch), `host` pointers are
+ *     ordinary or pinned host memory owned by the caller; the library allocates no device memory
+ *     of its own and never frees the caller's;
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - vx_build_table1 / vx_sort_match_table2 only ENQUEUE work on that stream and return; errors
+ *     raised on the device (slack overflow) surface as VX_ERR_OVERFLOW at the next synchronising
+ *     call (vx_read_tables, vx_get_stats, vx_synchronize);
+ *   - handles are independent: the key travels as a kernel parameter (constant bank), not in a
+ *     module-global __constant__, so plots with different keys can coexist.
+ *
+ * External record formats (reading A1, A4, A12; SURVEY.md 8(c) Step 5)
+ *   NONCE_SIZE = 4 for K <= 32, 5 for 33 <= K <= 40
+ *   Table-1 record: nonce[NONCE_SIZE] little-endian || hash[8]  (the 8 digest bytes, = H big-endian)
+ *   Table-2 record: nonce1[NONCE_SIZE] || nonce2[NONCE_SIZE], little-endian
+ *   offsets: uint64, CSR style, (number of buckets + 1) entries, in records.
+ */
+#ifndef VX_H_
+#define VX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vx_plot vx_plot; /* opaque; owns only host metadata */
+
+typedef enum {
+    VX_OK = 0,
+    VX_ERR_ARG = -1,       /* bad argument (NULL, K out of range, bucket range reversed ...)      */
+    VX_ERR_STATE = -2,     /* call out of order (e.g. sort_match before build, read before bind)  */
+    VX_ERR_WORKSPACE = -3, /* bound workspace smaller than vx_workspace_bytes / misaligned        */
+    VX_ERR_CUDA = -4,      /* a CUDA runtime call failed; text in vx_last_error                    */
+    VX_ERR_OVERFLOW = -5,  /* a partition's slack or the Table-2 capacity overflowed on the device */
+    VX_ERR_RANGE = -6,     /* bucket range outside [0, 2^B] or records_capacity too small          */
+    VX_ERR_UNSUPPORTED = -7 /* K valid per the paper's problem but not built yet (K > 32)          */
+} vx_status;
+
+/* Device bytes the caller must provide for a plot of this K (B = 24 buckets bits, the paper's
+ * setting).  0 if K is out of range.  Host-only arithmetic, no CUDA call. */
+size_t vx_workspace_bytes(uint32_t K);
+/* Same for a test-only bucket_bits (see vx_plot_create_ex). */
+size_t vx_workspace_bytes_ex(uint32_t K, uint32_t bucket_bits);
+
+/* Create a plot handle for 2^K nonces under a 256-bit key (host pointer, copied).  K in 1..32
+ * (33..40 return VX_ERR_UNSUPPORTED until the 5-byte-nonce path lands).  PAPER.md L41-43. */
+vx_status vx_plot_create(uint32_t K, const uint8_t key[32], vx_plot **out);
+/* Test-only: bucket_bits B in 1..24 instead of 24 (dense buckets at tiny K, reading A7). */
+vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out);
+
+/* Attach caller-owned device memory (>= vx_workspace_bytes, 256-byte aligned).  The workspace
+ * holds Table 1, Table 2, their offsets and the partition scratch for the life of the plot. */
+vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes);
+
+/* Stage 1: hash every nonce and place its record
+ * into its hash-prefix partition in HBM.  Enqueues only.  After it, Table 1 is resident in HBM as
+ * 2^P coarse hash-prefix buckets (P = max(K-12, 0) capped at B); the split of each coarse bucket
+ * into its 2^(B-P) buckets is an in-shared-memory counting step of the fused kernel below (or
+ * of vx_read_tables when Table 1 is read before vx_sort_match_table2).  See DESIGN.md "hierarchy". */
+vx_status vx_build_table1(vx_plot *p, void *cuda_stream);
+
+/* Stage 2 (rows a6-a8; "fused ... single GPU kernel"): for every bucket, stage it in
+ * shared memory, sort by (H, n), apply the match predicate, write the sorted bucket to the final
+ * Table 1 (reading A14) and the matches to Table 2, with exact CSR offsets for both. Enqueues only. */
+vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream);
+
+/* Copy the buckets [bucket_begin, bucket_end) of table 1 or 2 to HOST memory in the external
+ * format.  Synchronises the plot's stream.  offsets_out (may be NULL) receives
+ * bucket_end - bucket_begin + 1 entries relative to the first record of bucket_begin.
+ * records_out == NULL only queries *records_bytes.  records_capacity is in bytes.
+ * Table 1 may be read after vx_build_table1 alone (in-bucket order then unspecified, reading A9);
+ * Table 2 only after vx_sort_match_table2. */
+vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t bucket_end,
+                         uint64_t *offsets_out, void *records_out, size_t records_capacity,
+                         size_t *records_bytes);
+
+/* Device-side view for callers that keep the tables on the GPU (all pointers are DEVICE pointers
+ * into the bound workspace; valid after vx_sort_match_table2 has completed). */
+vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
+                           const void **dev_t2_records, const uint64_t **dev_t2_offsets);
+
+/* Synchronises; any output pointer may be NULL.  max_bucket = largest Table-1 bucket. */
+vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, uint32_t *max_bucket);
+
+/* Wait for the plot's enqueued work and report device-raised errors. */
+vx_status vx_synchronize(vx_plot *p);
+
+/* Hash kernel alone (7 build-plan step 3): H(n) for
+ * n in [nonce_begin, nonce_begin + count) written as uint64 to dev_hashes[count].  Enqueues only. */
+vx_status vx_hash_range(vx_plot *p, uint64_t nonce_begin, uint64_t count, uint64_t *dev_hashes,
+                        void *cuda_stream);
+
+/* Measurement aid for the ALU roofline: hashes `count` nonces starting at 0 and folds them into
+ * one xor word per thread block (dev_sink[grid] uint64) -- the BLAKE3 stage with no table traffic. */
+vx_status vx_hash_sink(vx_plot *p, uint64_t count, uint64_t *dev_sink, size_t sink_words,
+                       void *cuda_stream);
+
+/* Plot geometry, for tests and the bench report.  Any pointer may be NULL. */
+vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uint32_t *nonce_size,
+                       uint32_t *partition_bits, uint32_t *partition_capacity, uint64_t *t2_capacity);
+
+const char *vx_last_error(const vx_plot *p); /* never NULL; includes cudaGetErrorString text */
+const char *vx_status_string(vx_status s);
+void vx_free(vx_plot *p);                     /* frees the handle, never the workspace */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VX_H_ */

@@ -1,0 +1,9 @@
+"""paper_2606_14007_b200 -- B200-native VaultxGPU plotting hot path.
+
+BLAKE3 keyed hash of every nonce -> bucketed Table 1 in HBM -> fused per-bucket sort + match ->
+Table 2.  All arithmetic runs in the hand-written sm_100a kernels of
+`libvx.so` (C ABI: include/vx.h); this package is the thin ctypes binding.  PyTorch provides the
+device memory and streams only.  There is no CPU fallback.
+"""
+from .binding import (Plot, VxError, build_library, hash_range, library_path, load_library,  # noqa: F401
+                      workspace_bytes, EXPORTS)

@@ -1,0 +1,240 @@
+"""ctypes binding of libvx.so with the same names as include/vx.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI.  PyTorch supplies the
+device workspace (a uint8 CUDA tensor) and the stream.  If the library or a CUDA device is
+missing, calls raise: nothing here computes on the CPU.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+VX_OK = 0
+STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",
+          -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED"}
+
+#: every symbol include/vx.h declares
+EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_plot_create", "vx_plot_create_ex",
+           "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_read_tables",
+           "vx_device_tables", "vx_get_stats", "vx_synchronize", "vx_hash_range", "vx_hash_sink",
+           "vx_plot_info", "vx_last_error", "vx_status_string", "vx_free"]
+
+_u64 = ctypes.c_uint64
+_u32 = ctypes.c_uint32
+_vp = ctypes.c_void_p
+_sz = ctypes.c_size_t
+
+
+class VxError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"{STATUS.get(status, status)}: {text}")
+        self.status = status
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def build_library(force: bool = False) -> str:
+    return _build.build(force=force)
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Load (building first if the sources are newer) libvx.so.  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.is_stale():
+        path = _build.build()
+    L = ctypes.CDLL(path)
+    L.vx_workspace_bytes.restype = _sz
+    L.vx_workspace_bytes.argtypes = [_u32]
+    L.vx_workspace_bytes_ex.restype = _sz
+    L.vx_workspace_bytes_ex.argtypes = [_u32, _u32]
+    L.vx_plot_create.restype = ctypes.c_int
+    L.vx_plot_create.argtypes = [_u32, ctypes.c_char_p, ctypes.POINTER(_vp)]
+    L.vx_plot_create_ex.restype = ctypes.c_int
+    L.vx_plot_create_ex.argtypes = [_u32, ctypes.c_char_p, _u32, ctypes.POINTER(_vp)]
+    L.vx_plot_bind.restype = ctypes.c_int
+    L.vx_plot_bind.argtypes = [_vp, _vp, _sz]
+    L.vx_build_table1.restype = ctypes.c_int
+    L.vx_build_table1.argtypes = [_vp, _vp]
+    L.vx_sort_match_table2.restype = ctypes.c_int
+    L.vx_sort_match_table2.argtypes = [_vp, _vp]
+    L.vx_read_tables.restype = ctypes.c_int
+    L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
+    L.vx_device_tables.restype = ctypes.c_int
+    L.vx_device_tables.argtypes = [_vp] + [ctypes.POINTER(_vp)] * 4
+    L.vx_get_stats.restype = ctypes.c_int
+    L.vx_get_stats.argtypes = [_vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64), ctypes.POINTER(_u32)]
+    L.vx_synchronize.restype = ctypes.c_int
+    L.vx_synchronize.argtypes = [_vp]
+    L.vx_hash_range.restype = ctypes.c_int
+    L.vx_hash_range.argtypes = [_vp, _u64, _u64, _vp, _vp]
+    L.vx_hash_sink.restype = ctypes.c_int
+    L.vx_hash_sink.argtypes = [_vp, _u64, _vp, _sz, _vp]
+    L.vx_plot_info.restype = ctypes.c_int
+    L.vx_plot_info.argtypes = [_vp] + [ctypes.POINTER(_u32)] * 5 + [ctypes.POINTER(_u64)]
+    L.vx_last_error.restype = ctypes.c_char_p
+    L.vx_last_error.argtypes = [_vp]
+    L.vx_status_string.restype = ctypes.c_char_p
+    L.vx_status_string.argtypes = [ctypes.c_int]
+    L.vx_free.restype = None
+    L.vx_free.argtypes = [_vp]
+    _lib = L
+    return L
+
+
+def workspace_bytes(K: int, bucket_bits: int = 24) -> int:
+    return int(load_library().vx_workspace_bytes_ex(K, bucket_bits))
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+class Plot:
+    """One plot (K, key): vx_plot_create + vx_plot_bind on a torch-owned workspace."""
+
+    def __init__(self, K: int, key: bytes, bucket_bits: int = 24, device="cuda:0", workspace=None):
+        import torch
+        if len(key) != 32:
+            raise ValueError("key must be 32 bytes")
+        self._L = load_library()
+        self._h = _vp()
+        st = self._L.vx_plot_create_ex(K, bytes(key), bucket_bits, ctypes.byref(self._h))
+        if st != VX_OK:
+            raise VxError(st, f"vx_plot_create_ex(K={K}, bucket_bits={bucket_bits})")
+        self.K, self.bucket_bits = K, bucket_bits
+        info = [_u32() for _ in range(5)]
+        t2cap = _u64()
+        self._L.vx_plot_info(self._h, *[ctypes.byref(x) for x in info], ctypes.byref(t2cap))
+        self.nonce_size = info[2].value
+        self.partition_bits = info[3].value
+        self.partition_capacity = info[4].value
+        self.t2_capacity = t2cap.value
+        self.rec1_bytes = self.nonce_size + 8
+        self.rec2_bytes = 2 * self.nonce_size
+        need = int(self._L.vx_workspace_bytes_ex(K, bucket_bits))
+        if not torch.cuda.is_available():
+            self.free()
+            raise VxError(-4, "no CUDA device: libvx has no CPU fallback")
+        self.device = torch.device(device)
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device=self.device)
+        self.workspace = workspace
+        self.workspace_bytes = need
+        with torch.cuda.device(self.device):
+            self._check(self._L.vx_plot_bind(self._h, workspace.data_ptr(), workspace.numel()))
+
+    # -- plumbing -------------------------------------------------------------------------------
+    def _check(self, st: int):
+        if st != VX_OK:
+            raise VxError(st, self._L.vx_last_error(self._h).decode())
+
+    def free(self):
+        if getattr(self, "_h", None):
+            self._L.vx_free(self._h)
+            self._h = None
+        self.workspace = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.free()
+
+    # -- the hot path ---------------------------------------------------------------------------
+    def build_table1(self, stream=None):
+        self._check(self._L.vx_build_table1(self._h, _stream_ptr(stream)))
+
+    def sort_match_table2(self, stream=None):
+        self._check(self._L.vx_sort_match_table2(self._h, _stream_ptr(stream)))
+
+    def synchronize(self):
+        self._check(self._L.vx_synchronize(self._h))
+
+    def get_stats(self):
+        t1, t2, mb = _u64(), _u64(), _u32()
+        self._check(self._L.vx_get_stats(self._h, ctypes.byref(t1), ctypes.byref(t2), ctypes.byref(mb)))
+        return {"t1_records": t1.value, "t2_records": t2.value, "max_bucket": mb.value}
+
+    def read_tables(self, table: int, bucket_begin: int = 0, bucket_end: int | None = None,
+                    records_out: np.ndarray | None = None):
+        """(offsets uint64[nb+1] relative to the range, records uint8[...]) copied to the host."""
+        if bucket_end is None:
+            bucket_end = 1 << self.bucket_bits
+        nb = bucket_end - bucket_begin
+        offsets = np.empty(max(nb, 0) + 1, dtype=np.uint64)
+        need = _sz()
+        self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
+                                           offsets.ctypes.data, None, 0, ctypes.byref(need)))
+        if records_out is None:
+            records_out = np.empty(need.value, dtype=np.uint8)
+        assert records_out.dtype == np.uint8 and records_out.flags.c_contiguous
+        self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
+                                           offsets.ctypes.data, records_out.ctypes.data,
+                                           records_out.nbytes, ctypes.byref(need)))
+        return offsets, records_out[:need.value]
+
+    def read_tables_into(self, table: int, bucket_begin: int, bucket_end: int,
+                         offsets_ptr: int, records_ptr: int, records_capacity: int) -> int:
+        """Raw-pointer form (e.g. pinned torch tensors): returns the record bytes written."""
+        need = _sz()
+        self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
+                                           offsets_ptr, records_ptr, records_capacity, ctypes.byref(need)))
+        return need.value
+
+    def device_tables(self):
+        ptrs = [_vp() for _ in range(4)]
+        self._check(self._L.vx_device_tables(self._h, *[ctypes.byref(x) for x in ptrs]))
+        return [x.value for x in ptrs]
+
+    def hash_range(self, nonce_begin: int, count: int, stream=None):
+        """H(n) for n in [nonce_begin, nonce_begin+count) as a torch int64 CUDA tensor (bit pattern of u64)."""
+        import torch
+        out = torch.empty(count, dtype=torch.int64, device=self.device)
+        with torch.cuda.device(self.device):
+            self._check(self._L.vx_hash_range(self._h, nonce_begin, count, out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def hash_sink(self, count: int, sink, stream=None):
+        self._check(self._L.vx_hash_sink(self._h, count, sink.data_ptr(), sink.numel(), _stream_ptr(stream)))
+
+
+def hash_range(K: int, key: bytes, nonce_begin: int, count: int):
+    """Convenience: H(n) for a nonce range without building tables (no workspace needed)."""
+    import torch
+    L = load_library()
+    h = _vp()
+    st = L.vx_plot_create(K, bytes(key), ctypes.byref(h))
+    if st != VX_OK:
+        raise VxError(st, f"vx_plot_create(K={K})")
+    try:
+        if not torch.cuda.is_available():
+            raise VxError(-4, "no CUDA device: libvx has no CPU fallback")
+        out = torch.empty(count, dtype=torch.int64, device="cuda:0")
+        st = L.vx_hash_range(h, nonce_begin, count, out.data_ptr(), _stream_ptr(None))
+        if st != VX_OK:
+            raise VxError(st, L.vx_last_error(h).decode())
+        torch.cuda.synchronize()
+        return out
+    finally:
+        L.vx_free(h)

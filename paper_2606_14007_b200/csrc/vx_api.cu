@@ -1,0 +1,340 @@
+// vx_api.cu -- the C ABI of libvx (include/vx.h): host-side state machine, workspace plan,
+// launches and read-back.  No device memory is allocated here: the workspace is the caller's.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/vx.h"
+#include "vx_internal.h"
+
+enum VxState { VX_CREATED = 0, VX_BOUND = 1, VX_BUILT = 2, VX_MATCHED = 3 };
+
+struct vx_plot {
+    VxGeom g;
+    VxHashConst hc;
+    uint8_t key[32];
+    uint8_t *ws;
+    size_t ws_bytes;
+    VxState state;
+    bool t1_materialised;   // the 2^B-bucket view of Table 1 exists in the workspace
+    cudaStream_t stream;    // stream of the last enqueue
+    int num_sms;
+    char err[512];
+};
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ------------------------------------------------------------------------------ geometry
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B)
+{
+    memset(g, 0, sizeof *g);
+    if (K < 1 || K > 40 || B < 1 || B > 24) return false;
+    if (K > B + VX_MAX_MEAN_BUCKET_LOG) return false;
+    g->K = K; g->B = B;
+    g->nonce_size = K <= 32 ? 4 : 5;                       // reading A1
+    g->pb = K > VX_TILE_LOG ? K - VX_TILE_LOG : 0;
+    if (g->pb > B) return false;                           // cannot happen while K - B <= 9
+    g->fb = B - g->pb;
+    g->N = 1ull << K; g->P = 1ull << g->pb; g->NB = 1ull << B;
+    const uint64_t mean = g->N >> g->pb;
+    uint64_t cap;
+    if (g->pb == 0) cap = mean;                            // the single partition holds everything
+    else cap = mean + (uint64_t)ceil(9.0 * sqrt((double)mean)) + 32;   // Poisson tail, 9 sigma
+    cap = (cap + 31) & ~(uint64_t)31;
+    if (cap > VX_MAX_CAP) return false;
+    g->cap = (uint32_t)cap;
+    // |T2| ~ 2^K (1 - 2^(B-K-1)) for K >= B, 2^(2K-1-B) below; sd ~ sqrt: 2^K + slack is ample
+    g->t2_cap = g->N + (1u << 16);
+    g->rec1_bytes = g->nonce_size + 8;
+    g->rec2_bytes = 2 * g->nonce_size;
+    size_t o = 0;
+    g->off_ctrl = o;      o = align256(o + sizeof(VxCtrl));
+    g->off_cursor = o;    o = align256(o + g->P * 4);
+    g->off_part_base = o; o = align256(o + (g->P + 1) * 8);
+    g->off_status = o;    o = align256(o + g->P * 8);
+    g->off_part_hi = o;   o = align256(o + g->P * (size_t)g->cap * 8);
+    g->off_part_lo = o;   o = align256(o + g->P * (size_t)g->cap * 4);
+    g->off_t1_off = o;    o = align256(o + (g->NB + 1) * 8);
+    g->off_t2_off = o;    o = align256(o + (g->NB + 1) * 8);
+    g->off_t1_rec = o;    o = align256(o + g->N * (size_t)g->rec1_bytes);
+    g->off_t2_rec = o;    o = align256(o + g->t2_cap * (size_t)g->rec2_bytes);
+    g->total = o;
+    return true;
+}
+
+// ------------------------------------------------------------------------------ host fold
+// BLAKE3 G function on the host, used once per plot for the three nonce-independent columns of
+// round 1 (message words 2..7 are zero for a nonce of at most 5 bytes).  BLAKE3 spec 2.2.
+static uint32_t h_rotr(uint32_t x, int r) { return (x >> r) | (x << (32 - r)); }
+static void h_g0(uint32_t &a, uint32_t &b, uint32_t &c, uint32_t &d)
+{
+    a = a + b;  d = h_rotr(d ^ a, 16);  c = c + d;  b = h_rotr(b ^ c, 12);
+    a = a + b;  d = h_rotr(d ^ a, 8);   c = c + d;  b = h_rotr(b ^ c, 7);
+}
+
+void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_size)
+{
+    const uint32_t iv[4] = {VX_IV0, VX_IV1, VX_IV2, VX_IV3};
+    for (int i = 0; i < 8; i++)
+        hc->k[i] = (uint32_t)key[4 * i] | ((uint32_t)key[4 * i + 1] << 8) |
+                   ((uint32_t)key[4 * i + 2] << 16) | ((uint32_t)key[4 * i + 3] << 24);
+    hc->s04 = hc->k[0] + hc->k[4];
+    hc->block_len = nonce_size;
+    // v12 = v13 = 0 (counter), v14 = block_len, v15 = flags
+    const uint32_t tail[4] = {0u, 0u, nonce_size, VX_FLAGS};
+    for (int c = 1; c < 4; c++) {
+        uint32_t a = hc->k[c], b = hc->k[4 + c], cc = iv[c], d = tail[c];
+        h_g0(a, b, cc, d);
+        hc->col[4 * (c - 1) + 0] = a;
+        hc->col[4 * (c - 1) + 1] = b;
+        hc->col[4 * (c - 1) + 2] = cc;
+        hc->col[4 * (c - 1) + 3] = d;
+    }
+}
+
+// ------------------------------------------------------------------------------ helpers
+static vx_status fail(vx_plot *p, vx_status s, const char *what)
+{
+    if (p) snprintf(p->err, sizeof p->err, "%s: %s", vx_status_string(s), what);
+    return s;
+}
+
+static vx_status fail_cuda(vx_plot *p, cudaError_t e, const char *what)
+{
+    if (p) snprintf(p->err, sizeof p->err, "VX_ERR_CUDA: %s: %s", what, cudaGetErrorString(e));
+    return VX_ERR_CUDA;
+}
+
+static vx_status sync_and_check(vx_plot *p)
+{
+    cudaError_t e = cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaStreamSynchronize");
+    if (p->state >= VX_BUILT) {
+        VxCtrl c;
+        e = cudaMemcpy(&c, p->ws + p->g.off_ctrl, sizeof c, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(ctrl)");
+        if (c.flags & VX_FLAG_PART_OVERFLOW)
+            return fail(p, VX_ERR_OVERFLOW, "a stage-1 partition exceeded its slack capacity");
+        if (c.flags & VX_FLAG_T2_OVERFLOW)
+            return fail(p, VX_ERR_OVERFLOW, "Table 2 exceeded its capacity");
+    }
+    return VX_OK;
+}
+
+// ------------------------------------------------------------------------------ the ABI
+extern "C" {
+
+const char *vx_status_string(vx_status s)
+{
+    switch (s) {
+    case VX_OK: return "VX_OK";
+    case VX_ERR_ARG: return "VX_ERR_ARG";
+    case VX_ERR_STATE: return "VX_ERR_STATE";
+    case VX_ERR_WORKSPACE: return "VX_ERR_WORKSPACE";
+    case VX_ERR_CUDA: return "VX_ERR_CUDA";
+    case VX_ERR_OVERFLOW: return "VX_ERR_OVERFLOW";
+    case VX_ERR_RANGE: return "VX_ERR_RANGE";
+    case VX_ERR_UNSUPPORTED: return "VX_ERR_UNSUPPORTED";
+    }
+    return "VX_ERR_?";
+}
+
+size_t vx_workspace_bytes_ex(uint32_t K, uint32_t bucket_bits)
+{
+    VxGeom g;
+    if (!vx_geom_init(&g, K, bucket_bits) || g.nonce_size != 4) return 0;
+    return g.total;
+}
+
+size_t vx_workspace_bytes(uint32_t K) { return vx_workspace_bytes_ex(K, 24); }
+
+vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out)
+{
+    if (!out) return VX_ERR_ARG;
+    *out = NULL;
+    if (!key) return VX_ERR_ARG;
+    VxGeom g;
+    if (!vx_geom_init(&g, K, bucket_bits)) return VX_ERR_ARG;
+    if (g.nonce_size != 4) return VX_ERR_UNSUPPORTED;
+    vx_plot *p = new (std::nothrow) vx_plot;
+    if (!p) return VX_ERR_ARG;
+    memset(p, 0, sizeof *p);
+    p->g = g;
+    memcpy(p->key, key, 32);
+    vx_hash_const_init(&p->hc, key, g.nonce_size);
+    p->state = VX_CREATED;
+    snprintf(p->err, sizeof p->err, "VX_OK");
+    *out = p;
+    return VX_OK;
+}
+
+vx_status vx_plot_create(uint32_t K, const uint8_t key[32], vx_plot **out)
+{
+    return vx_plot_create_ex(K, key, 24, out);
+}
+
+vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes)
+{
+    if (!p || !dev_workspace) return fail(p, VX_ERR_ARG, "NULL plot or workspace");
+    if (((uintptr_t)dev_workspace & 255) != 0) return fail(p, VX_ERR_WORKSPACE, "workspace not 256-byte aligned");
+    if (bytes < p->g.total) return fail(p, VX_ERR_WORKSPACE, "workspace smaller than vx_workspace_bytes");
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaGetDevice (no CUDA device: there is no CPU fallback)");
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaGetDeviceProperties");
+    if (prop.major < 10) return fail(p, VX_ERR_CUDA, "libvx is built for sm_100a only");
+    p->num_sms = prop.multiProcessorCount;
+    e = vx_stage2_configure();
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute(stage 2 shared memory)");
+    p->ws = (uint8_t *)dev_workspace;
+    p->ws_bytes = bytes;
+    p->state = VX_BOUND;
+    p->t1_materialised = false;
+    p->stream = 0;
+    return VX_OK;
+}
+
+vx_status vx_build_table1(vx_plot *p, void *cuda_stream)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_BOUND) return fail(p, VX_ERR_STATE, "vx_build_table1 before vx_plot_bind");
+    p->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = vx_launch_stage1(p->g, p->hc, p->ws, p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "stage 1 launch");
+    p->state = VX_BUILT;
+    p->t1_materialised = false;
+    return VX_OK;
+}
+
+vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "vx_sort_match_table2 before vx_build_table1");
+    p->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = vx_launch_stage2(p->g, p->ws, true, p->num_sms, p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "stage 2 launch");
+    p->state = VX_MATCHED;
+    p->t1_materialised = true;
+    return VX_OK;
+}
+
+vx_status vx_synchronize(vx_plot *p)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_BOUND) return fail(p, VX_ERR_STATE, "vx_synchronize before vx_plot_bind");
+    return sync_and_check(p);
+}
+
+vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t bucket_end,
+                         uint64_t *offsets_out, void *records_out, size_t records_capacity,
+                         size_t *records_bytes)
+{
+    if (!p) return VX_ERR_ARG;
+    if (table != 1 && table != 2) return fail(p, VX_ERR_ARG, "table must be 1 or 2");
+    if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "vx_read_tables before vx_build_table1");
+    if (table == 2 && p->state < VX_MATCHED)
+        return fail(p, VX_ERR_STATE, "Table 2 read before vx_sort_match_table2");
+    if (bucket_begin > bucket_end || bucket_end > p->g.NB)
+        return fail(p, VX_ERR_RANGE, "bucket range outside [0, 2^B]");
+    if (!p->t1_materialised) {
+        // Table 1 read after stage 1 alone: split the partitions into buckets now (no matching)
+        cudaError_t e = vx_launch_stage2(p->g, p->ws, false, p->num_sms, p->stream);
+        if (e != cudaSuccess) return fail_cuda(p, e, "stage 2 (bucket view) launch");
+        p->t1_materialised = true;
+    }
+    vx_status s = sync_and_check(p);
+    if (s != VX_OK) return s;
+    const uint8_t *off_dev = p->ws + (table == 1 ? p->g.off_t1_off : p->g.off_t2_off);
+    const uint8_t *rec_dev = p->ws + (table == 1 ? p->g.off_t1_rec : p->g.off_t2_rec);
+    const size_t rb = table == 1 ? p->g.rec1_bytes : p->g.rec2_bytes;
+    const uint64_t nb = bucket_end - bucket_begin;
+    uint64_t first = 0, last = 0;
+    cudaError_t e = cudaMemcpy(&first, off_dev + bucket_begin * 8, 8, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(&last, off_dev + bucket_end * 8, 8, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(offsets ends)");
+    const size_t need = (size_t)(last - first) * rb;
+    if (records_bytes) *records_bytes = need;
+    if (offsets_out) {
+        e = cudaMemcpy(offsets_out, off_dev + bucket_begin * 8, (nb + 1) * 8, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(offsets)");
+        for (uint64_t i = 0; i <= nb; i++) offsets_out[i] -= first;
+    }
+    if (!records_out) return VX_OK;
+    if (records_capacity < need) return fail(p, VX_ERR_RANGE, "records_capacity too small");
+    if (need) {
+        e = cudaMemcpy(records_out, rec_dev + (size_t)first * rb, need, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(records)");
+    }
+    return VX_OK;
+}
+
+vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
+                           const void **dev_t2_records, const uint64_t **dev_t2_offsets)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_MATCHED) return fail(p, VX_ERR_STATE, "vx_device_tables before vx_sort_match_table2");
+    if (dev_t1_records) *dev_t1_records = p->ws + p->g.off_t1_rec;
+    if (dev_t1_offsets) *dev_t1_offsets = (const uint64_t *)(p->ws + p->g.off_t1_off);
+    if (dev_t2_records) *dev_t2_records = p->ws + p->g.off_t2_rec;
+    if (dev_t2_offsets) *dev_t2_offsets = (const uint64_t *)(p->ws + p->g.off_t2_off);
+    return VX_OK;
+}
+
+vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, uint32_t *max_bucket)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "vx_get_stats before vx_build_table1");
+    vx_status s = sync_and_check(p);
+    if (s != VX_OK) return s;
+    VxCtrl c;
+    cudaError_t e = cudaMemcpy(&c, p->ws + p->g.off_ctrl, sizeof c, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(ctrl)");
+    uint64_t t1 = 0;
+    e = cudaMemcpy(&t1, p->ws + p->g.off_part_base + p->g.P * 8, 8, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(part_base)");
+    if (t1_records) *t1_records = t1;
+    if (t2_records) *t2_records = p->state >= VX_MATCHED ? c.t2_total : 0;
+    if (max_bucket) *max_bucket = p->t1_materialised ? c.max_bucket : 0;
+    return VX_OK;
+}
+
+vx_status vx_hash_range(vx_plot *p, uint64_t nonce_begin, uint64_t count, uint64_t *dev_hashes,
+                        void *cuda_stream)
+{
+    if (!p || (!dev_hashes && count)) return fail(p, VX_ERR_ARG, "NULL argument");
+    cudaError_t e = vx_launch_hash_range(p->g, p->hc, nonce_begin, count, dev_hashes, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "hash_range launch");
+    return VX_OK;
+}
+
+vx_status vx_hash_sink(vx_plot *p, uint64_t count, uint64_t *dev_sink, size_t sink_words, void *cuda_stream)
+{
+    if (!p || !dev_sink) return fail(p, VX_ERR_ARG, "NULL argument");
+    cudaError_t e = vx_launch_hash_sink(p->g, p->hc, count, dev_sink, sink_words, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "hash_sink launch");
+    return VX_OK;
+}
+
+vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uint32_t *nonce_size,
+                       uint32_t *partition_bits, uint32_t *partition_capacity, uint64_t *t2_capacity)
+{
+    if (!p) return VX_ERR_ARG;
+    if (K) *K = p->g.K;
+    if (bucket_bits) *bucket_bits = p->g.B;
+    if (nonce_size) *nonce_size = p->g.nonce_size;
+    if (partition_bits) *partition_bits = p->g.pb;
+    if (partition_capacity) *partition_capacity = p->g.cap;
+    if (t2_capacity) *t2_capacity = p->g.t2_cap;
+    return VX_OK;
+}
+
+const char *vx_last_error(const vx_plot *p) { return p ? p->err : "VX_ERR_ARG: NULL plot"; }
+
+void vx_free(vx_plot *p) { delete p; }
+
+} // extern "C"

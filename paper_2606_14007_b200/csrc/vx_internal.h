@@ -1,0 +1,66 @@
+// vx_internal.h -- geometry, workspace plan and launch wrappers shared by the .cu files of libvx.
+// Not part of the public ABI (that is include/vx.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "vx_blake3.cuh"
+
+// ---------------------------------------------------------------------------------- geometry
+// Hierarchical bucketing: stage 1 scatters records into 2^pb coarse
+// hash-prefix partitions of ~2^VX_TILE_LOG records each (they fit one CTA's shared memory);
+// stage 2 splits a partition into its 2^fb buckets (fb = B - pb) with a shared-memory
+// distribution sort over VX_BIN_BITS more hash bits (about one record per bin).
+#define VX_TILE_LOG 12          // log2 of the mean records per partition
+#define VX_BIN_BITS 12          // bins per partition in stage 2 = 2^VX_BIN_BITS
+#define VX_NBINS (1u << VX_BIN_BITS)
+#define VX_S2_THREADS 512
+#define VX_S2_ITEMS 10          // VX_S2_THREADS * VX_S2_ITEMS >= max partition capacity
+#define VX_MAX_CAP (VX_S2_THREADS * VX_S2_ITEMS)
+#define VX_MAX_MEAN_BUCKET_LOG 9 // K - B <= 9  (mean bucket <= 512 records, BASELINE.json K=33)
+
+struct VxGeom {
+    uint32_t K, B, nonce_size;
+    uint32_t pb;   // partition bits: partition = H >> (64 - pb)
+    uint32_t fb;   // bucket bits inside a partition, B - pb
+    uint32_t cap;  // partition capacity in records (mean + slack, multiple of 32)
+    uint64_t N;    // 2^K
+    uint64_t P;    // 2^pb
+    uint64_t NB;   // 2^B
+    uint64_t t2_cap; // Table-2 capacity in records
+    uint32_t rec1_bytes, rec2_bytes;
+    // workspace carve-up (byte offsets, each 256-aligned)
+    size_t off_ctrl, off_cursor, off_part_base, off_status;
+    size_t off_part_hi, off_part_lo;
+    size_t off_t1_off, off_t2_off, off_t1_rec, off_t2_rec;
+    size_t total;
+};
+
+// device-resident control block (first bytes of the workspace)
+struct VxCtrl {
+    uint32_t ticket;      // stage-2 tile dispenser
+    uint32_t flags;       // bit 0: partition slack overflow, bit 1: Table-2 capacity overflow
+    uint32_t max_bucket;  // largest Table-1 bucket seen by stage 2
+    uint32_t pad0;
+    unsigned long long t2_total;  // number of Table-2 records
+    unsigned long long pad1;
+};
+#define VX_FLAG_PART_OVERFLOW 1u
+#define VX_FLAG_T2_OVERFLOW 2u
+
+// returns false if (K, B) is not a supported geometry
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B);
+
+// host fold of the nonce-independent part of round 1 (vx_blake3.cuh)
+void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_size);
+
+// ---------------------------------------------------------------------------------- launches
+cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st);
+cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, int num_sms, cudaStream_t st);
+cudaError_t vx_launch_hash_range(const VxGeom &g, const VxHashConst &hc, uint64_t nonce_begin,
+                                 uint64_t count, uint64_t *dev_hashes, cudaStream_t st);
+cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t count,
+                                uint64_t *dev_sink, size_t sink_words, cudaStream_t st);
+cudaError_t vx_stage2_configure(void); // opt in to the large dynamic shared memory once
+size_t vx_stage2_smem_bytes(const VxGeom &g);

@@ -1,0 +1,190 @@
+// vx_stage1.cu -- stage 1 of the plot: BLAKE3 keyed hash of every nonce + scatter of the
+// (nonce, H) record into its hash-prefix partition in HBM.
+//
+// PAPER.md L81 (III-A): "a custom Blake3 CUDA kernel launches one thread per nonce across the full
+// 2^k nonce space, hashing each nonce independently and inserting the resulting nonce-hash pair
+// into its corresponding bucket in GPU VRAM using atomic operations"; L91 (III-B): "atomically
+// claims a slot in the corresponding bucket using atomicAdd".  SURVEY.md 8(a) rows a1-a5.
+//
+// What differs from the paper's kernel: the atomic append targets 2^pb
+// coarse partitions (pb = K - 12), not 2^24 buckets, so the set of partially written 32-byte
+// sectors (one or two per partition and array) stays far below the 126 MB L2 and every sector
+// reaches HBM exactly once, fully written; records are SoA (u64 H, u32 nonce) so both stores are
+// naturally aligned; several nonces per thread keep the atomics' latency off the ALU pipe.
+#include "vx_internal.h"
+
+#define VX_S1_THREADS 256
+#define VX_S1_NPT 4
+
+template <bool NONCE5>
+__global__ void __launch_bounds__(VX_S1_THREADS)
+vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t pb, uint32_t cap,
+                  uint64_t *__restrict__ part_hi, uint32_t *__restrict__ part_lo,
+                  uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
+{
+    const uint64_t base = (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
+    uint64_t H[VX_S1_NPT];
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
+        H[k] = vx_blake3_h<NONCE5>(hc, (uint32_t)n, (uint32_t)(n >> 32));
+    }
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
+        if (n < N) {
+            const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
+            const uint32_t slot = atomicAdd(&cursor[p], 1u);
+            if (slot < cap) {
+                const uint64_t at = (uint64_t)p * cap + slot;
+                part_hi[at] = H[k];
+                part_lo[at] = (uint32_t)n;
+            } else {
+                atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
+            }
+        }
+    }
+}
+
+// Exclusive prefix sum of the clamped partition counts: part_base[p] = number of records in
+// partitions < p, part_base[P] = total.  One CTA; P <= 2^20 so this is a few tens of microseconds.
+#define VX_SCAN_THREADS 1024
+#define VX_SCAN_ITEMS 16
+__global__ void __launch_bounds__(VX_SCAN_THREADS)
+vx_k_partition_scan(const uint32_t *__restrict__ cursor, uint32_t cap, uint64_t P,
+                    unsigned long long *__restrict__ part_base)
+{
+    __shared__ unsigned long long s_warp[32];
+    __shared__ unsigned long long s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (uint64_t chunk = 0; chunk < P; chunk += (uint64_t)VX_SCAN_THREADS * VX_SCAN_ITEMS) {
+        const uint64_t i0 = chunk + (uint64_t)tid * VX_SCAN_ITEMS;
+        uint32_t c[VX_SCAN_ITEMS];
+        unsigned long long sum = 0;
+#pragma unroll
+        for (int k = 0; k < VX_SCAN_ITEMS; k++) {
+            c[k] = (i0 + k < P) ? min(cursor[i0 + k], cap) : 0u;
+            sum += c[k];
+        }
+        unsigned long long incl = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long o = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += o;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        unsigned long long wbase = 0, total = 0;
+        {
+            unsigned long long w = s_warp[lane];   // 32 warps exactly
+            unsigned long long wi = w;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned long long o = __shfl_up_sync(0xffffffffu, wi, d);
+                if (lane >= d) wi += o;
+            }
+            wbase = __shfl_sync(0xffffffffu, wi - w, warp);
+            total = __shfl_sync(0xffffffffu, wi, 31);
+        }
+        unsigned long long run = s_carry + wbase + (incl - sum);
+#pragma unroll
+        for (int k = 0; k < VX_SCAN_ITEMS; k++) {
+            if (i0 + k < P) part_base[i0 + k] = run;
+            run += c[k];
+        }
+        __syncthreads();
+        if (tid == 0) s_carry += total;
+        __syncthreads();
+    }
+    if (tid == 0) part_base[P] = s_carry;
+}
+
+// ----------------------------------------------------------------------------- hash alone
+template <bool NONCE5>
+__global__ void __launch_bounds__(VX_S1_THREADS)
+vx_k_hash_range(const __grid_constant__ VxHashConst hc, uint64_t nonce_begin, uint64_t count,
+                uint64_t *__restrict__ out)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * VX_S1_THREADS + threadIdx.x;
+    if (i < count) {
+        const uint64_t n = nonce_begin + i;
+        out[i] = vx_blake3_h<NONCE5>(hc, (uint32_t)n, (uint32_t)(n >> 32));
+    }
+}
+
+// the BLAKE3 stage with no table traffic: xor-fold of every hash into one word per CTA
+template <bool NONCE5>
+__global__ void __launch_bounds__(VX_S1_THREADS)
+vx_k_hash_sink(const __grid_constant__ VxHashConst hc, uint64_t count, uint64_t *__restrict__ sink)
+{
+    const uint64_t base = (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
+    uint64_t x = 0;
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
+        const uint64_t h = vx_blake3_h<NONCE5>(hc, (uint32_t)n, (uint32_t)(n >> 32));
+        x ^= (n < count) ? h : 0ull;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) x ^= __shfl_xor_sync(0xffffffffu, x, d);
+    __shared__ uint64_t s[VX_S1_THREADS / 32];
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint64_t y = 0;
+        for (int w = 0; w < VX_S1_THREADS / 32; w++) y ^= s[w];
+        sink[blockIdx.x] = y;
+    }
+}
+
+// ----------------------------------------------------------------------------- launches
+cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st)
+{
+    VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
+    uint32_t *cursor = (uint32_t *)(ws + g.off_cursor);
+    cudaError_t e = cudaMemsetAsync(ctrl, 0, sizeof(VxCtrl), st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(cursor, 0, g.P * sizeof(uint32_t), st);
+    if (e != cudaSuccess) return e;
+    const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
+    const uint64_t grid = (g.N + per_cta - 1) / per_cta;
+    uint64_t *hi = (uint64_t *)(ws + g.off_part_hi);
+    uint32_t *lo = (uint32_t *)(ws + g.off_part_lo);
+    if (g.nonce_size == 5)
+        vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, hi, lo, cursor, ctrl);
+    else
+        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, hi, lo, cursor, ctrl);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap, g.P,
+                                                       (unsigned long long *)(ws + g.off_part_base));
+    return cudaGetLastError();
+}
+
+cudaError_t vx_launch_hash_range(const VxGeom &g, const VxHashConst &hc, uint64_t nonce_begin,
+                                 uint64_t count, uint64_t *dev_hashes, cudaStream_t st)
+{
+    if (count == 0) return cudaSuccess;
+    const uint64_t grid = (count + VX_S1_THREADS - 1) / VX_S1_THREADS;
+    if (g.nonce_size == 5)
+        vx_k_hash_range<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, nonce_begin, count, dev_hashes);
+    else
+        vx_k_hash_range<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, nonce_begin, count, dev_hashes);
+    return cudaGetLastError();
+}
+
+cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t count,
+                                uint64_t *dev_sink, size_t sink_words, cudaStream_t st)
+{
+    const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
+    const uint64_t grid = (count + per_cta - 1) / per_cta;
+    if (grid == 0) return cudaSuccess;
+    if (grid > sink_words) return cudaErrorInvalidValue;
+    if (g.nonce_size == 5)
+        vx_k_hash_sink<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, count, dev_sink);
+    else
+        vx_k_hash_sink<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, count, dev_sink);
+    return cudaGetLastError();
+}

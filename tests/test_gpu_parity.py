@@ -1,0 +1,201 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Bit-exact: everything here is integer work.
+
+Tolerance: none (north_star: "GPU results must be bit-exact against the oracle, comparing bucket
+contents after canonical ordering").
+"""
+import numpy as np
+import pytest
+
+import oracle
+import vx_inputs
+from vx_testlib import bucket_ids, canon_t1, canon_t2, decode_t1, decode_t2, oracle_tables
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def vx():
+    import paper_2606_14007_b200 as m
+    m.load_library()
+    return m
+
+
+def u64(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+# ------------------------------------------------------------------ hash kernel alone (a2-a4)
+@pytest.mark.parametrize("K,seed", [(20, 1), (27, 27), (31, 31), (32, 5)])
+def test_hash_range_vs_oracle(vx, K, seed):
+    key = vx_inputs.key_from_seed(seed)
+    N = 1 << K
+    for begin, count in ((0, 70001), (N - 4099, 4099), (N // 2 - 17, 1025)):
+        got = u64(vx.hash_range(K, key, begin, count))
+        want = oracle.hash_range(key, 4, begin, count)
+        assert np.array_equal(got, want)
+
+
+def test_hash_range_vs_blake3_library(vx):
+    blake3 = pytest.importorskip("blake3")
+    key = vx_inputs.key_from_seed(31)
+    got = u64(vx.hash_range(31, key, (1 << 31) - 300, 300))
+    for i in range(300):
+        n = (1 << 31) - 300 + i
+        want = int.from_bytes(blake3.blake3(n.to_bytes(4, "little"), key=key).digest(8), "big")
+        assert int(got[i]) == want
+
+
+def test_hash_worked_values(vx):
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "blake3_worked_values.txt")
+    for ln in open(path):
+        if ln.startswith("#") or not ln.strip():
+            continue
+        K, seed, n, hx = ln.split()
+        if int(K) > 32:
+            continue
+        got = u64(vx.hash_range(int(K), vx_inputs.key_from_seed(int(seed)), int(n), 1))
+        assert f"{int(got[0]):016x}" == hx
+
+
+# ------------------------------------------------------------------ full tables, small K
+def run_plot(vx, K, key, B):
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    # Table 1 straight after stage 1: bucket order unspecified (A9) -> canonicalise
+    off_b, raw_b = plot.read_tables(1)
+    plot.sort_match_table2()
+    off1, raw1 = plot.read_tables(1)
+    off2, raw2 = plot.read_tables(2)
+    stats = plot.get_stats()
+    nsize = plot.nonce_size
+    plot.free()
+    return (off_b, raw_b), (off1, raw1), (off2, raw2), stats, nsize
+
+
+FULL_CASES = [
+    # (K, B, seed): tiny brute-force geometries, one partition, ragged sizes, several partitions
+    (4, 2, 3), (8, 4, 1), (10, 6, 2), (12, 8, 1), (12, 12, 7), (10, 24, 8),
+    (13, 8, 4), (14, 9, 5), (16, 12, 1), (16, 7, 6), (18, 12, 9), (18, 24, 3), (20, 24, 1),
+    (21, 12, 2), (22, 24, 22),
+]
+
+
+@pytest.mark.parametrize("K,B,seed", FULL_CASES)
+def test_tables_bit_exact_vs_oracle(vx, K, B, seed):
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    (off_b, raw_b), (off1, raw1), (off2, raw2), stats, nsize = run_plot(vx, K, key, B)
+
+    # Table 1 after build only
+    assert np.array_equal(off_b, o_off)
+    nb, hb = canon_t1(off_b, *decode_t1(raw_b, nsize))
+    assert np.array_equal(nb, o_non) and np.array_equal(hb, o_has)
+
+    # Table 1 after sort+match: sorted in place, byte-exact with the oracle's serialisation
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(nsize, o_non, o_has))
+
+    # Table 2: offsets exact; bucket contents equal after canonical (n1, n2) ordering
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    # and as raw bytes: the multiset of 8-byte external records is the oracle's
+    assert nsize == 4
+    assert np.array_equal(np.sort(raw2.view(np.uint64)),
+                          np.sort(oracle.serialize_t2(nsize, o_n1, o_n2).view(np.uint64)))
+
+    sizes = np.diff(o_off)
+    assert stats == {"t1_records": 1 << K, "t2_records": len(o_n1), "max_bucket": int(sizes.max())}
+
+
+def test_ranged_reads(vx):
+    K, B, seed = 16, 12, 1
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    plot.sort_match_table2()
+    for b0, b1 in ((0, 1), (5, 5), (100, 1000), (4095, 4096), (0, 4096)):
+        off, raw = plot.read_tables(1, b0, b1)
+        lo, hi = int(o_off[b0]), int(o_off[b1])
+        assert np.array_equal(off, o_off[b0:b1 + 1] - o_off[b0])
+        assert np.array_equal(raw, oracle.serialize_t1(4, o_non[lo:hi], o_has[lo:hi]))
+        off, raw = plot.read_tables(2, b0, b1)
+        lo, hi = int(o_t2o[b0]), int(o_t2o[b1])
+        assert np.array_equal(off, o_t2o[b0:b1 + 1] - o_t2o[b0])
+        g1, g2 = canon_t2(off, *decode_t2(raw, 4))
+        assert np.array_equal(g1, o_n1[lo:hi]) and np.array_equal(g2, o_n2[lo:hi])
+    with pytest.raises(vx.VxError) as ei:
+        plot.read_tables(1, 10, 5)
+    assert ei.value.status == -6
+    with pytest.raises(vx.VxError):
+        plot.read_tables(2, 0, 4097)
+    with pytest.raises(vx.VxError) as ei:
+        plot.read_tables(1, 0, 4096, records_out=np.empty(8, dtype=np.uint8))
+    assert ei.value.status == -6
+    plot.free()
+
+
+def test_state_machine_and_rebuild(vx):
+    import torch
+    K, B = 14, 9
+    key = vx_inputs.key_from_seed(5)
+    plot = vx.Plot(K, key, B)
+    with pytest.raises(vx.VxError) as ei:
+        plot.sort_match_table2()
+    assert ei.value.status == -2
+    plot.build_table1()
+    with pytest.raises(vx.VxError) as ei:
+        plot.read_tables(2)
+    assert ei.value.status == -2
+    plot.sort_match_table2()
+    a = plot.read_tables(2)
+    # a second full run on a side stream gives the same tables (buffers fully reset)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        plot.build_table1()
+        plot.sort_match_table2()
+    b = plot.read_tables(2)
+    assert np.array_equal(a[0], b[0])
+    assert np.array_equal(np.sort(a[1].view(np.uint64)), np.sort(b[1].view(np.uint64)))
+    with pytest.raises(vx.VxError) as ei:
+        vx.Plot(K, key, B, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
+    assert ei.value.status == -3
+    plot.free()
+
+
+def test_two_plots_with_different_keys_coexist(vx):
+    K, B = 13, 8
+    k1, k2 = vx_inputs.key_from_seed(101), vx_inputs.key_from_seed(202)
+    p1, p2 = vx.Plot(K, k1, B), vx.Plot(K, k2, B)
+    p1.build_table1(); p2.build_table1()
+    p1.sort_match_table2(); p2.sort_match_table2()
+    for p, k in ((p1, k1), (p2, k2)):
+        o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, k, B)
+        off1, raw1 = p.read_tables(1)
+        assert np.array_equal(off1, o_off) and np.array_equal(raw1, oracle.serialize_t1(4, o_non, o_has))
+        off2, raw2 = p.read_tables(2)
+        g1, g2 = canon_t2(off2, *decode_t2(raw2, 4))
+        assert np.array_equal(off2, o_t2o) and np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    p1.free(); p2.free()
+
+
+# ------------------------------------------------------------------ K = 24: mean one record per bucket
+def test_K24_full_parity(vx):
+    K, B = 24, 24
+    key = vx_inputs.config_key(K)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    plot.sort_match_table2()
+    off1, raw1 = plot.read_tables(1)
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(4, o_non, o_has))
+    off2, raw2 = plot.read_tables(2)
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, 4))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    assert plot.get_stats()["t2_records"] == 8386097        # tests/golden/match_counts.txt
+    plot.free()
