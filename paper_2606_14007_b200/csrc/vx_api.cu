@@ -55,8 +55,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B)
     g->off_cursor = o;    o = align256(o + g->P * 4);
     g->off_part_base = o; o = align256(o + (g->P + 1) * 8);
     g->off_status = o;    o = align256(o + g->P * 8);
-    g->off_part_hi = o;   o = align256(o + g->P * (size_t)g->cap * 8);
-    g->off_part_lo = o;   o = align256(o + g->P * (size_t)g->cap * 4);
+    g->off_part = o;      o = align256(o + g->P * (size_t)g->cap * 16);
     g->off_t1_off = o;    o = align256(o + (g->NB + 1) * 8);
     g->off_t2_off = o;    o = align256(o + (g->NB + 1) * 8);
     g->off_t1_rec = o;    o = align256(o + g->N * (size_t)g->rec1_bytes);

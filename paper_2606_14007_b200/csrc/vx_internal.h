@@ -32,7 +32,7 @@ struct VxGeom {
     uint32_t rec1_bytes, rec2_bytes;
     // workspace carve-up (byte offsets, each 256-aligned)
     size_t off_ctrl, off_cursor, off_part_base, off_status;
-    size_t off_part_hi, off_part_lo;
+    size_t off_part;   // partition records: uint4 {H lo, H hi, nonce lo, nonce hi} per record
     size_t off_t1_off, off_t2_off, off_t1_rec, off_t2_rec;
     size_t total;
 };

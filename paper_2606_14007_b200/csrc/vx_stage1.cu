@@ -8,9 +8,10 @@
 //
 // What differs from the paper's kernel: the atomic append targets 2^pb
 // coarse partitions (pb = K - 12), not 2^24 buckets, so the set of partially written 32-byte
-// sectors (one or two per partition and array) stays far below the 126 MB L2 and every sector
-// reaches HBM exactly once, fully written; records are SoA (u64 H, u32 nonce) so both stores are
-// naturally aligned; several nonces per thread keep the atomics' latency off the ALU pipe.
+// sectors (one per partition) stays far below the 126 MB L2 and is merged there; a record is ONE
+// aligned 16-byte store {H, nonce} because scattered stores on B200 are bound by request count
+// (~50 G/s once the write frontier spans more pages than the TLB reaches), not by bytes;
+// several nonces per thread keep the atomics' latency off the ALU pipe.
 #include "vx_internal.h"
 
 #define VX_S1_THREADS 256
@@ -19,8 +20,8 @@
 template <bool NONCE5>
 __global__ void __launch_bounds__(VX_S1_THREADS)
 vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t pb, uint32_t cap,
-                  uint64_t *__restrict__ part_hi, uint32_t *__restrict__ part_lo,
-                  uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
+                  uint4 *__restrict__ part, uint32_t *__restrict__ cursor,
+                  VxCtrl *__restrict__ ctrl)
 {
     const uint64_t base = (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
     uint64_t H[VX_S1_NPT];
@@ -36,9 +37,9 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t p
             const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
             const uint32_t slot = atomicAdd(&cursor[p], 1u);
             if (slot < cap) {
-                const uint64_t at = (uint64_t)p * cap + slot;
-                part_hi[at] = H[k];
-                part_lo[at] = (uint32_t)n;
+                // one 16-byte store per record: scattered stores are bound by requests, not bytes
+                part[(uint64_t)p * cap + slot] =
+                    make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)n, (uint32_t)(n >> 32));
             } else {
                 atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
             }
@@ -150,12 +151,11 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
     if (e != cudaSuccess) return e;
     const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
     const uint64_t grid = (g.N + per_cta - 1) / per_cta;
-    uint64_t *hi = (uint64_t *)(ws + g.off_part_hi);
-    uint32_t *lo = (uint32_t *)(ws + g.off_part_lo);
+    uint4 *part = (uint4 *)(ws + g.off_part);
     if (g.nonce_size == 5)
-        vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, hi, lo, cursor, ctrl);
+        vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, part, cursor, ctrl);
     else
-        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, hi, lo, cursor, ctrl);
+        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, part, cursor, ctrl);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap, g.P,

@@ -24,8 +24,7 @@
 #include "vx_internal.h"
 
 struct VxS2Params {
-    const uint64_t *part_hi;
-    const uint32_t *part_lo;
+    const uint4 *part;           // stage-1 partition records {H lo, H hi, nonce lo, nonce hi}
     const uint32_t *cursor;
     const unsigned long long *part_base;
     unsigned long long *status;
@@ -148,8 +147,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
         const uint32_t cnt = min(q.cursor[tile], q.cap);
         const unsigned long long base1 = q.part_base[tile];
-        const uint64_t *hi = q.part_hi + (size_t)tile * q.cap;
-        const uint32_t *lo = q.part_lo + (size_t)tile * q.cap;
+        const uint4 *src = q.part + (size_t)tile * q.cap;
 
         // ---- 1. load + bin count -------------------------------------------------------------
         uint64_t key[ITEMS];
@@ -157,8 +155,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 #pragma unroll
         for (int it = 0; it < ITEMS; it++) {
             const uint32_t idx = it * THREADS + tid;
-            key[it] = idx < cnt ? __ldg(hi + idx) : 0ull;
-            non[it] = idx < cnt ? __ldg(lo + idx) : 0u;
+            const uint4 r = idx < cnt ? __ldg(src + idx) : make_uint4(0u, 0u, 0u, 0u);
+            key[it] = ((uint64_t)r.y << 32) | r.x;
+            non[it] = r.z;
         }
 #pragma unroll
         for (int it = 0; it < ITEMS; it++) {
@@ -313,8 +312,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, int nu
     e = cudaMemsetAsync(ws + g.off_status, 0, g.P * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     VxS2Params q;
-    q.part_hi = (const uint64_t *)(ws + g.off_part_hi);
-    q.part_lo = (const uint32_t *)(ws + g.off_part_lo);
+    q.part = (const uint4 *)(ws + g.off_part);
     q.cursor = (const uint32_t *)(ws + g.off_cursor);
     q.part_base = (const unsigned long long *)(ws + g.off_part_base);
     q.status = (unsigned long long *)(ws + g.off_status);
