@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- the plotting hot path on N B200s, one JSON line.
+
+A "step" is one pass of the whole hot path over one plot: vx_build_table1 (BLAKE3 keyed hash of
+all 2^K nonces + bucket construction) followed by vx_sort_match_table2 (fused per-bucket sort +
+match, Table 1 sorted + Table 2 written), through the C ABI.
+
+  metric  nonces hashed + bucketed + sorted + matched per second for the whole plot (BASELINE.json:
+          "nonces hashed+bucketed/s; end-to-end K=31 Table1+Table2 plot time (s), 1 B200"); the plot
+          seconds and the per-stage nonces/s ride along in "plot_seconds" and "stages".
+  value   device-timed, tables stay resident in HBM (the input is (K, key); nothing else exists).
+  e2e     the same through the C ABI with HOST buffers: every step also copies the key in and
+          streams Table 2 + its offsets to pinned host memory with vx_read_tables (the paper's
+          egress, minus the disk), inside the timed region.
+  roofline  the dominant kernel of the step; "stages" carries both kernels.
+  cpu_baseline  the oracle as it stands on this box's host cores, bounded sample (N=1 only).
+
+--impl reference times the CPU oracle itself (this tier's reference arm).
+N > 1: independent plots, one per rank (the path partitions by plot; no data-path collective),
+"scaling": "weak"; launched by torch.distributed.run.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "nonces hashed+bucketed+sorted+matched per second (whole Table1+Table2 plot)"
+UNIT = "nonces/s"
+BUCKET_BITS = 24
+# algorithmic work per nonce: SURVEY.md 8(d)
+ALU_OPS_PER_NONCE = 415            # xor / rotate / byte-swap lane-ops that need the ALU pipe
+S2_BYTES_PER_NONCE = 12 + 12 + 8   # read record, write sorted record, write ~1 Table-2 record
+S1_BYTES_PER_NONCE = 12            # write the record once
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
+                "source": "MEASURED_PEAKS.json"}
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [x.strip() for x in r.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = [x for x in sm if x >= 0.5 * max(sm)] or sm
+        return {"sm_mhz": statistics.median(busy), "sm_max_mhz": max(mx), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def make_config(K: int):
+    import vx_inputs
+    idx = {20: 0, 27: 1, 29: 2, 31: 3, 33: 4}.get(K, "-")
+    return {"workload": f"K={K} plot: 2^{K} nonces, key SplitMix64({vx_inputs.seed_for_K(K)}), 2^24 buckets "
+                        f"(BASELINE.json configs[{idx}])",
+            "K": K, "bucket_bits": BUCKET_BITS, "plots_per_gpu": 1,
+            "l2": "inputs larger than L2 (tens of GB of tables are rewritten every step)"}
+
+
+# --------------------------------------------------------------------------- CPU oracle legs
+def oracle_plot_seconds(K: int, seed: int):
+    """One whole plot with the oracle, single thread: (seconds, stage1 s, stage2 s, |T2|)."""
+    import oracle
+    import vx_inputs
+    key = vx_inputs.key_from_seed(seed)
+    t0 = time.perf_counter()
+    off, non, has = oracle.table1(K, key, BUCKET_BITS)
+    t1 = time.perf_counter()
+    t2o, n1, n2 = oracle.table2(K, off, non, has, 1)
+    t2 = time.perf_counter()
+    return t2 - t0, t1 - t0, t2 - t1, len(n1)
+
+
+def cpu_baseline(sample_K: int):
+    total, s1, s2, m = oracle_plot_seconds(sample_K, sample_K)
+    return {"value": (1 << sample_K) / total, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"whole plot at K={sample_K} (2^{sample_K} nonces, key SplitMix64({sample_K}), B=24), "
+                      f"single thread: Table 1 {s1:.2f} s + Table 2 {s2:.2f} s, |T2|={m}",
+            "seconds": total}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    K = args.ref_K
+    for _ in range(args.warmup):
+        oracle_plot_seconds(K, K)
+    times = []
+    for _ in range(args.steps):
+        times.append(oracle_plot_seconds(K, K)[0])
+    total = sum(times)
+    value = args.steps * (1 << K) / total
+    sample = (f"each step = one whole oracle plot at K={K} (2^{K} nonces, B=24), single thread; "
+              f"bounded sample of the K={args.K} workload")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": make_config(args.K),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------- the CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2606_14007_b200 as vx
+    import vx_inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K = args.K
+    # independent plots: rank r plots under key SplitMix64(seed_for_K + 1000 r)
+    key = vx_inputs.key_from_seed(vx_inputs.seed_for_K(K) + 1000 * rank)
+    plot = vx.Plot(K, key, BUCKET_BITS, device=dev)
+    N = 1 << K
+    stream = torch.cuda.current_stream()
+
+    def step(evs=None):
+        if evs: evs[0].record(stream)
+        plot.build_table1(stream)
+        if evs: evs[1].record(stream)
+        plot.sort_match_table2(stream)
+        if evs: evs[2].record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    stats = plot.get_stats()
+
+    # ---- device-timed region -------------------------------------------------------------
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    for i in range(args.steps):
+        step(evs[i])
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = evs[0][0].elapsed_time(evs[-1][2])
+    s1_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    s2_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    plot.synchronize()
+
+    # ---- end to end through the C ABI with host buffers -----------------------------------
+    # per step: key (32 B) in; Table 2 + its offsets out, streamed through a pinned staging buffer
+    nb = 1 << BUCKET_BITS
+    chunks = args.e2e_chunks
+    per = nb // chunks
+    rec_cap = int(1.25 * plot.rec2_bytes * (N // chunks)) + (1 << 20)
+    pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
+    pinned_off = torch.empty(per + 1, dtype=torch.int64, pin_memory=True)
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    d2h = 0
+
+    def e2e_step():
+        nonlocal d2h
+        p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace)  # key -> kernel params
+        p2.build_table1(stream)
+        p2.sort_match_table2(stream)
+        moved = 0
+        for c in range(chunks):
+            moved += p2.read_tables_into(2, c * per, (c + 1) * per, pinned_off.data_ptr(),
+                                         pinned_rec.data_ptr(), rec_cap) + (per + 1) * 8
+        d2h = moved
+        p2.free()
+
+    e2e_step()                      # warm the pinned path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+
+    # ---- max over ranks -------------------------------------------------------------------
+    vals = torch.tensor([total_ms, e2e_s, statistics.mean(s1_ms), statistics.mean(s2_ms)],
+                        dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+    total_ms, e2e_s, s1, s2 = [float(x) for x in vals.tolist()]
+    ms_per_step = total_ms / args.steps
+
+    if rank == 0:
+        peaks = measured_peaks()
+        alu_peak = 148 * 4 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12     # T lane-ops/s on the ALU pipe
+        r1 = {"kernel": "vx_k_hash_scatter", "bound": "alu", "achieved": ALU_OPS_PER_NONCE * N / (s1 * 1e-3) / 1e12,
+              "peak": alu_peak, "unit": "Tlaneop/s", "traffic": None, "ms": s1,
+              "hbm_algorithmic_GBps": S1_BYTES_PER_NONCE * N / (s1 * 1e-3) / 1e9}
+        r1["frac"] = r1["achieved"] / r1["peak"]
+        r2 = {"kernel": "vx_k_sort_match", "bound": "hbm", "achieved": S2_BYTES_PER_NONCE * N / (s2 * 1e-3) / 1e9,
+              "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": None, "ms": s2}
+        r2["frac"] = r2["achieved"] / r2["peak"]
+        dominant = dict(r1 if s1 >= s2 else r2)
+        dominant["peak_source"] = peaks["source"] + (" (hbm_gbs, burst copy)" if dominant["bound"] == "hbm"
+                                                     else " (sm_max_mhz x 148 SM x 4 SMSP x 16 ALU lanes; DESIGN.md)")
+        line = {
+            "metric": METRIC, "value": world * N / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64",
+            "data": "synthetic",
+            "config": make_config(K),
+            "plot_seconds": ms_per_step * 1e-3, "workspace_GB": plot.workspace_bytes / 1e9,
+            "stages": {"build_table1": {"ms": s1, "nonces_per_s": N / (s1 * 1e-3), "roofline": r1},
+                       "sort_match_table2": {"ms": s2, "nonces_per_s": N / (s2 * 1e-3), "roofline": r2}},
+            "table_stats": stats,
+            "roofline": {k: dominant[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel", "peak_source")},
+            "e2e": {"value": world * N / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 32,
+                    "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
+                    "what": "vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2 + vx_read_tables(Table 2, "
+                            f"{chunks} bucket ranges) into pinned host memory"},
+            "gpu_launches": 3 * args.steps,
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args.cpu_K)
+        print(json.dumps(line), flush=True)
+    plot.free()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--K", type=int, default=31, help="plot size; 31 = the configuration the metric is quoted on")
+    ap.add_argument("--cpu-K", dest="cpu_K", type=int, default=24, help="oracle sample size for cpu_baseline")
+    ap.add_argument("--ref-K", dest="ref_K", type=int, default=22, help="oracle sample size per --impl reference step")
+    ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=2)
+    ap.add_argument("--e2e-chunks", dest="e2e_chunks", type=int, default=32)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        print("bench.py: note: warmup < 3 breaks the timing rules", file=sys.stderr)
+    if args.impl == "reference":
+        return run_reference(args)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1:
+            # convenience: relaunch under torch.distributed.run
+            cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                   "--master-addr", "127.0.0.1", "--master-port", "29541", os.path.abspath(__file__)] + sys.argv[1:]
+            return subprocess.call(cmd)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
