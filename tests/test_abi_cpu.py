@@ -33,8 +33,8 @@ def test_workspace_bytes_arithmetic():
     a, b = vx.workspace_bytes(27), vx.workspace_bytes(28)
     assert 0 < a < b
     # K=31: partitions + Table 1 (25.77 GB) + Table 2 (17.2 GB) + offsets fits one B200
-    assert 60e9 < vx.workspace_bytes(31) < 80e9
-    assert vx.workspace_bytes(32) < 150e9
+    assert 60e9 < vx.workspace_bytes(31) < 90e9
+    assert vx.workspace_bytes(32) < 175e9
     assert vx.workspace_bytes(16, 12) > 0 and vx.workspace_bytes(16, 4) == 0
 
 
