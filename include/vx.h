@@ -69,7 +69,8 @@ vx_status vx_plot_create(uint32_t K, const uint8_t key[32], vx_plot **out);
 vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out);
 
 /* Attach caller-owned device memory (>= vx_workspace_bytes, 256-byte aligned).  The workspace
- * holds Table 1, Table 2, their offsets and the partition scratch for the life of the plot. */
+ * holds Table 1 (the partition array), Table 2, their offsets, the look-back state and a small
+ * export staging area for the life of the plot. */
 vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes);
 
 /* Stage 1: hash every nonce and place its record
@@ -80,8 +81,9 @@ vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes);
 vx_status vx_build_table1(vx_plot *p, void *cuda_stream);
 
 /* Stage 2 (rows a6-a8; "fused ... single GPU kernel"): for every bucket, stage it in
- * shared memory, sort by (H, n), apply the match predicate, write the sorted bucket to the final
- * Table 1 (reading A14) and the matches to Table 2, with exact CSR offsets for both. Enqueues only. */
+ * shared memory, sort by (H, n), apply the match predicate, write the sorted bucket back to
+ * Table 1 in place (reading A14) and the matches to Table 2, with exact CSR offsets for both.
+ * Enqueues only. */
 vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream);
 
 /* Copy the buckets [bucket_begin, bucket_end) of table 1 or 2 to HOST memory in the external
@@ -95,9 +97,27 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
                          size_t *records_bytes);
 
 /* Device-side view for callers that keep the tables on the GPU (all pointers are DEVICE pointers
- * into the bound workspace; valid after vx_sort_match_table2 has completed). */
+ * into the bound workspace; valid after vx_sort_match_table2 has completed; any may be NULL).
+ *   Table 2: dev_t2_records = external 2*NONCE_SIZE-byte records, contiguous; dev_t2_offsets =
+ *     uint64[2^B + 1] CSR offsets in records.
+ *   Table 1 stays where stage 1 put it and is sorted IN PLACE (reading A14): dev_t1_records is the
+ *     partition array of 16-byte records {uint32 H low, H high, nonce low, nonce high}, 2^pb
+ *     partitions of `partition_capacity` slots each (vx_plot_info); partition q holds the buckets
+ *     [q << (B - pb), (q + 1) << (B - pb)) back to back, each sorted by (H, n).  dev_t1_offsets =
+ *     uint64[2^B + 1] CSR offsets in records (the numbering vx_read_tables uses) and
+ *     dev_partition_base = uint64[2^pb + 1], the CSR index of each partition's first record:
+ *     bucket b (partition q = b >> (B - pb)) starts at slot
+ *     q * partition_capacity + dev_t1_offsets[b] - dev_partition_base[q].
+ *   vx_read_tables converts to the external 12-byte Table-1 format on the way out. */
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
-                           const void **dev_t2_records, const uint64_t **dev_t2_offsets);
+                           const void **dev_t2_records, const uint64_t **dev_t2_offsets,
+                           const uint64_t **dev_partition_base);
+
+/* Test hooks.  VX_OPT_FORCE_EXACT_RANK (value != 0): the fused kernel always takes the exact
+ * (H, n) re-ranking path it otherwise takes only for a tile holding two equal 64-bit hashes
+ * (reading A10) -- results are identical by construction; tests use it to cover that path. */
+#define VX_OPT_FORCE_EXACT_RANK 1
+vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value);
 
 /* Synchronises; any output pointer may be NULL.  max_bucket = largest Table-1 bucket. */
 vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, uint32_t *max_bucket);

@@ -14,13 +14,15 @@ import numpy as np
 from . import build as _build
 
 VX_OK = 0
+VX_OPT_FORCE_EXACT_RANK = 1
 STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",
           -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED"}
 
 #: every symbol include/vx.h declares
 EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_plot_create", "vx_plot_create_ex",
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_read_tables",
-           "vx_device_tables", "vx_get_stats", "vx_synchronize", "vx_hash_range", "vx_hash_sink",
+           "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_synchronize", "vx_hash_range",
+           "vx_hash_sink",
            "vx_plot_info", "vx_last_error", "vx_status_string", "vx_free"]
 
 _u64 = ctypes.c_uint64
@@ -72,7 +74,9 @@ def load_library() -> ctypes.CDLL:
     L.vx_read_tables.restype = ctypes.c_int
     L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
     L.vx_device_tables.restype = ctypes.c_int
-    L.vx_device_tables.argtypes = [_vp] + [ctypes.POINTER(_vp)] * 4
+    L.vx_device_tables.argtypes = [_vp] + [ctypes.POINTER(_vp)] * 5
+    L.vx_plot_set_option.restype = ctypes.c_int
+    L.vx_plot_set_option.argtypes = [_vp, ctypes.c_int, _u64]
     L.vx_get_stats.restype = ctypes.c_int
     L.vx_get_stats.argtypes = [_vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64), ctypes.POINTER(_u32)]
     L.vx_synchronize.restype = ctypes.c_int
@@ -202,8 +206,12 @@ class Plot:
                                            offsets_ptr, records_ptr, records_capacity, ctypes.byref(need)))
         return need.value
 
+    def set_option(self, option: int, value: int):
+        self._check(self._L.vx_plot_set_option(self._h, option, value))
+
     def device_tables(self):
-        ptrs = [_vp() for _ in range(4)]
+        """[t1 partition array, t1 offsets, t2 records, t2 offsets, partition base] device pointers."""
+        ptrs = [_vp() for _ in range(5)]
         self._check(self._L.vx_device_tables(self._h, *[ctypes.byref(x) for x in ptrs]))
         return [x.value for x in ptrs]
 

@@ -20,6 +20,7 @@ struct vx_plot {
     size_t ws_bytes;
     VxState state;
     bool t1_materialised;   // the 2^B-bucket view of Table 1 exists in the workspace
+    bool force_exact;       // VX_OPT_FORCE_EXACT_RANK
     cudaStream_t stream;    // stream of the last enqueue
     int num_sms;
     char err[512];
@@ -42,7 +43,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B)
     const uint64_t mean = g->N >> g->pb;
     uint64_t cap;
     if (g->pb == 0) cap = mean;                            // the single partition holds everything
-    else cap = mean + (uint64_t)ceil(9.0 * sqrt((double)mean)) + 32;   // Poisson tail, 9 sigma
+    else cap = mean + (uint64_t)ceil(8.0 * sqrt((double)mean));        // Poisson tail, 8 sigma
     cap = (cap + 31) & ~(uint64_t)31;
     if (cap > VX_MAX_CAP) return false;
     g->cap = (uint32_t)cap;
@@ -58,8 +59,10 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B)
     g->off_part = o;      o = align256(o + g->P * (size_t)g->cap * 16);
     g->off_t1_off = o;    o = align256(o + (g->NB + 1) * 8);
     g->off_t2_off = o;    o = align256(o + (g->NB + 1) * 8);
-    g->off_t1_rec = o;    o = align256(o + g->N * (size_t)g->rec1_bytes);
     g->off_t2_rec = o;    o = align256(o + g->t2_cap * (size_t)g->rec2_bytes);
+    g->stage_bytes = g->N * (size_t)g->rec1_bytes;
+    if (g->stage_bytes > VX_STAGE_MAX_BYTES) g->stage_bytes = VX_STAGE_MAX_BYTES;
+    g->off_stage = o;     o = align256(o + g->stage_bytes);
     g->total = o;
     return true;
 }
@@ -215,7 +218,7 @@ vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream)
     if (!p) return VX_ERR_ARG;
     if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "vx_sort_match_table2 before vx_build_table1");
     p->stream = (cudaStream_t)cuda_stream;
-    cudaError_t e = vx_launch_stage2(p->g, p->ws, true, p->num_sms, p->stream);
+    cudaError_t e = vx_launch_stage2(p->g, p->ws, true, p->force_exact, p->num_sms, p->stream);
     if (e != cudaSuccess) return fail_cuda(p, e, "stage 2 launch");
     p->state = VX_MATCHED;
     p->t1_materialised = true;
@@ -242,14 +245,13 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
         return fail(p, VX_ERR_RANGE, "bucket range outside [0, 2^B]");
     if (!p->t1_materialised) {
         // Table 1 read after stage 1 alone: split the partitions into buckets now (no matching)
-        cudaError_t e = vx_launch_stage2(p->g, p->ws, false, p->num_sms, p->stream);
+        cudaError_t e = vx_launch_stage2(p->g, p->ws, false, p->force_exact, p->num_sms, p->stream);
         if (e != cudaSuccess) return fail_cuda(p, e, "stage 2 (bucket view) launch");
         p->t1_materialised = true;
     }
     vx_status s = sync_and_check(p);
     if (s != VX_OK) return s;
     const uint8_t *off_dev = p->ws + (table == 1 ? p->g.off_t1_off : p->g.off_t2_off);
-    const uint8_t *rec_dev = p->ws + (table == 1 ? p->g.off_t1_rec : p->g.off_t2_rec);
     const size_t rb = table == 1 ? p->g.rec1_bytes : p->g.rec2_bytes;
     const uint64_t nb = bucket_end - bucket_begin;
     uint64_t first = 0, last = 0;
@@ -265,23 +267,49 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
     }
     if (!records_out) return VX_OK;
     if (records_capacity < need) return fail(p, VX_ERR_RANGE, "records_capacity too small");
-    if (need) {
-        e = cudaMemcpy(records_out, rec_dev + (size_t)first * rb, need, cudaMemcpyDeviceToHost);
+    if (need == 0) return VX_OK;
+    if (table == 2) {
+        // Table 2 is resident in the external format: one contiguous copy
+        e = cudaMemcpy(records_out, p->ws + p->g.off_t2_rec + (size_t)first * rb, need, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(records)");
+        return VX_OK;
+    }
+    // Table 1 is resident as sorted buckets inside the partition array (16-byte internal records):
+    // gather + convert to the external format through the staging area, a chunk at a time
+    const uint64_t per = p->g.stage_bytes / rb;
+    for (uint64_t done = 0; done < last - first; done += per) {
+        const uint64_t n = (last - first - done) < per ? (last - first - done) : per;
+        e = vx_launch_export_t1(p->g, p->ws, first + done, n, p->stream);
+        if (e != cudaSuccess) return fail_cuda(p, e, "export launch");
+        e = cudaMemcpyAsync((uint8_t *)records_out + done * rb, p->ws + p->g.off_stage, n * rb,
+                            cudaMemcpyDeviceToHost, p->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(exported records)");
     }
     return VX_OK;
 }
 
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
-                           const void **dev_t2_records, const uint64_t **dev_t2_offsets)
+                           const void **dev_t2_records, const uint64_t **dev_t2_offsets,
+                           const uint64_t **dev_partition_base)
 {
     if (!p) return VX_ERR_ARG;
     if (p->state < VX_MATCHED) return fail(p, VX_ERR_STATE, "vx_device_tables before vx_sort_match_table2");
-    if (dev_t1_records) *dev_t1_records = p->ws + p->g.off_t1_rec;
+    if (dev_t1_records) *dev_t1_records = p->ws + p->g.off_part;
     if (dev_t1_offsets) *dev_t1_offsets = (const uint64_t *)(p->ws + p->g.off_t1_off);
     if (dev_t2_records) *dev_t2_records = p->ws + p->g.off_t2_rec;
     if (dev_t2_offsets) *dev_t2_offsets = (const uint64_t *)(p->ws + p->g.off_t2_off);
+    if (dev_partition_base) *dev_partition_base = (const uint64_t *)(p->ws + p->g.off_part_base);
     return VX_OK;
+}
+
+vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value)
+{
+    if (!p) return VX_ERR_ARG;
+    switch (option) {
+    case VX_OPT_FORCE_EXACT_RANK: p->force_exact = value != 0; return VX_OK;
+    }
+    return fail(p, VX_ERR_ARG, "unknown option");
 }
 
 vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, uint32_t *max_bucket)

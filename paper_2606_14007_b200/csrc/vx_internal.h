@@ -16,8 +16,9 @@
 #define VX_BIN_BITS 12          // bins per partition in stage 2 = 2^VX_BIN_BITS
 #define VX_NBINS (1u << VX_BIN_BITS)
 #define VX_S2_THREADS 512
-#define VX_S2_ITEMS 10          // VX_S2_THREADS * VX_S2_ITEMS >= max partition capacity
+#define VX_S2_ITEMS 9           // VX_S2_THREADS * VX_S2_ITEMS >= max partition capacity
 #define VX_MAX_CAP (VX_S2_THREADS * VX_S2_ITEMS)
+#define VX_STAGE_MAX_BYTES ((size_t)64 << 20) // Table-1 export staging (vx_read_tables)
 #define VX_MAX_MEAN_BUCKET_LOG 9 // K - B <= 9  (mean bucket <= 512 records, BASELINE.json K=33)
 
 struct VxGeom {
@@ -32,8 +33,10 @@ struct VxGeom {
     uint32_t rec1_bytes, rec2_bytes;
     // workspace carve-up (byte offsets, each 256-aligned)
     size_t off_ctrl, off_cursor, off_part_base, off_status;
-    size_t off_part;   // partition records: uint4 {H lo, H hi, nonce lo, nonce hi} per record
-    size_t off_t1_off, off_t2_off, off_t1_rec, off_t2_rec;
+    size_t off_part;   // partition records: uint4 {H lo, H hi, nonce lo, nonce hi} per record;
+                       // after stage 2 each partition is sorted: this IS the resident Table 1
+    size_t off_t1_off, off_t2_off, off_t2_rec;
+    size_t off_stage, stage_bytes;   // export staging for vx_read_tables(Table 1)
     size_t total;
 };
 
@@ -57,7 +60,10 @@ void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_s
 
 // ---------------------------------------------------------------------------------- launches
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st);
-cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, int num_sms, cudaStream_t st);
+cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool force_exact, int num_sms,
+                             cudaStream_t st);
+// external-format Table-1 records [first, first + count) of the CSR numbering -> ws + off_stage
+cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
 cudaError_t vx_launch_hash_range(const VxGeom &g, const VxHashConst &hc, uint64_t nonce_begin,
                                  uint64_t count, uint64_t *dev_hashes, cudaStream_t st);
 cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t count,

@@ -60,8 +60,10 @@ def test_hash_worked_values(vx):
 
 
 # ------------------------------------------------------------------ full tables, small K
-def run_plot(vx, K, key, B):
+def run_plot(vx, K, key, B, force_exact=False):
     plot = vx.Plot(K, key, B)
+    if force_exact:
+        plot.set_option(vx.VX_OPT_FORCE_EXACT_RANK, 1)
     plot.build_table1()
     # Table 1 straight after stage 1: bucket order unspecified (A9) -> canonicalise
     off_b, raw_b = plot.read_tables(1)
@@ -108,6 +110,51 @@ def test_tables_bit_exact_vs_oracle(vx, K, B, seed):
 
     sizes = np.diff(o_off)
     assert stats == {"t1_records": 1 << K, "t2_records": len(o_n1), "max_bucket": int(sizes.max())}
+
+
+@pytest.mark.parametrize("K,B,seed", [(12, 8, 1), (16, 7, 6), (18, 24, 3), (21, 12, 2)])
+def test_exact_rerank_path_gives_the_same_tables(vx, K, B, seed):
+    """The (H, n) re-ranking path the kernel takes when a tile holds two equal 64-bit hashes
+    (reading A10), forced on every tile: the tables must still be the oracle's."""
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    _, (off1, raw1), (off2, raw2), stats, nsize = run_plot(vx, K, key, B, force_exact=True)
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(nsize, o_non, o_has))
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+
+
+def test_device_tables_layout(vx):
+    """vx_device_tables: Table 1 sorted in place in the partition array, as include/vx.h states."""
+    import torch
+    K, B = 16, 12
+    key = vx_inputs.key_from_seed(1)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    plot.sort_match_table2()
+    plot.synchronize()
+    t1, t1o, t2, t2o, pbase = plot.device_tables()
+    ws = plot.workspace
+    base = ws.data_ptr()
+    P, cap = 1 << plot.partition_bits, plot.partition_capacity
+    part = ws[t1 - base: t1 - base + P * cap * 16].cpu().numpy().view(np.uint32).reshape(P, cap, 4)
+    pb = ws[pbase - base: pbase - base + (P + 1) * 8].cpu().numpy().view(np.uint64)
+    offs = ws[t1o - base: t1o - base + ((1 << B) + 1) * 8].cpu().numpy().view(np.uint64)
+    assert np.array_equal(offs, o_off)
+    fb = B - plot.partition_bits
+    for b in (0, 1, 77, 2048, 4095):
+        q = b >> fb
+        lo = int(offs[b] - pb[q]); hi = int(offs[b + 1] - pb[q])
+        rec = part[q, lo:hi]
+        H = (rec[:, 1].astype(np.uint64) << np.uint64(32)) | rec[:, 0].astype(np.uint64)
+        assert np.array_equal(H, o_has[int(o_off[b]):int(o_off[b + 1])])
+        assert np.array_equal(rec[:, 2].astype(np.uint64), o_non[int(o_off[b]):int(o_off[b + 1])])
+    t2r = ws[t2 - base: t2 - base + len(o_n1) * 8].cpu().numpy()
+    assert np.array_equal(np.sort(t2r.view(np.uint64)), np.sort(oracle.serialize_t2(4, o_n1, o_n2).view(np.uint64)))
+    plot.free()
 
 
 def test_ranged_reads(vx):
