@@ -112,7 +112,7 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
         unsigned long long s = VX_ST_INC;   // lanes before tile 0 count as "inclusive, value 0"
         if (idx >= 0) {
             s = vs[idx];
-            while ((s >> 62) == 0) { __nanosleep(20); s = vs[idx]; }
+            while ((s >> 62) == 0) { __nanosleep(100); s = vs[idx]; }
         }
         const unsigned incmask = __ballot_sync(VX_FULL, (s >> 62) == 2);
         unsigned long long v = s & VX_ST_VAL;
@@ -136,8 +136,8 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 {
     constexpr int CAPA = THREADS * ITEMS;               // allocated sorted positions
     extern __shared__ __align__(16) uint8_t vx_smem[];
-    uint64_t *keyS = (uint64_t *)vx_smem;               // CAPA sorted hashes
-    uint32_t *nonS = (uint32_t *)(keyS + CAPA);         // CAPA sorted nonces (low 32 bits)
+    uint64_t *keyS = (uint64_t *)vx_smem;               // CAPA sorted hashes + sentinel (+ pad)
+    uint32_t *nonS = (uint32_t *)(keyS + CAPA + 2);     // CAPA sorted nonces (low 32 bits)
     uint32_t *bins = nonS + CAPA;                       // VX_NBINS + 1 (+ pad)
     uint32_t *E = bins + VX_NBINS + 32;                 // CAPA + 1 (+ pad): match-count prefix
     __shared__ uint32_t s_warp[32];
@@ -154,104 +154,160 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
     for (;;) {
         __syncthreads();                                // previous tile fully drained
-        if (tid == 0) { s_tile = atomicAdd(&q.ctrl->ticket, 1u); s_tie = q.force_exact; }
-        for (int i = tid; i < (int)(VX_NBINS + 32) / 4; i += THREADS)
-            reinterpret_cast<uint4 *>(bins)[i] = make_uint4(0u, 0u, 0u, 0u);
-        __syncthreads();
-        const uint32_t tile = s_tile;
-        if (tile >= q.P) break;
-
-        const uint32_t cnt = min(q.cursor[tile], q.cap);
-        const unsigned long long base1 = q.part_base[tile];
-        uint4 *src = q.part + (size_t)tile * q.cap;
-
-        // ---- A. load + bin count ---------------------------------------------------------------
+        if (tid == 0) s_tile = atomicAdd(&q.ctrl->ticket, 1u);
+        // exact = rank by (H, n) with full compares; the fast pass ranks by H alone and is
+        // validated in phase E (a tile holding two equal hashes comes back for an exact pass)
+        uint32_t exact = q.force_exact | (q.do_match ^ 1u);
+        uint32_t tile, cnt;
+        unsigned long long base1;
+        uint4 *src;
         uint64_t key[ITEMS];
-        uint32_t non[ITEMS], sn[ITEMS];                 // sn: slot, later bin start | bin size << 16
-#pragma unroll
-        for (int it = 0; it < ITEMS; it++) {
-            const uint32_t idx = it * THREADS + tid;
-            const uint4 r = idx < cnt ? __ldcs(src + idx) : make_uint4(0u, 0u, 0u, 0u);
-            key[it] = ((uint64_t)r.y << 32) | r.x;
-            non[it] = r.z;
-        }
-#pragma unroll
-        for (int it = 0; it < ITEMS; it++) {
-            const uint32_t idx = it * THREADS + tid;
-            if (idx < cnt) sn[it] = atomicAdd(&bins[(uint32_t)(key[it] >> binshift) & (VX_NBINS - 1)], 1u);
-        }
-        __syncthreads();
-        // ---- B. scan -----------------------------------------------------------------------------
-        {
-            const uint32_t total = vx_block_exscan<THREADS, VX_NBINS / THREADS>(bins, s_warp);
-            if (tid == 0) bins[VX_NBINS] = total;
-        }
-        __syncthreads();
-        // ---- C. scatter to bin start + slot ---------------------------------------------------------
-#pragma unroll
-        for (int it = 0; it < ITEMS; it++) {
-            if (it * THREADS + wbase < cnt) {           // warp-uniform
-                const uint32_t idx = it * THREADS + tid;
-                if (idx < cnt) {
-                    const uint32_t b = (uint32_t)(key[it] >> binshift) & (VX_NBINS - 1);
-                    const uint32_t s = bins[b], e = bins[b + 1];
-                    const uint32_t pos = s + sn[it];
-                    keyS[pos] = key[it];
-                    nonS[pos] = non[it];
-                    sn[it] = s | ((e - s) << 16);
-                }
-            }
-        }
-        __syncthreads();
-        // ---- D. rank inside multi-record bins (by H; ties flagged) ------------------------------------
-#pragma unroll
-        for (int it = 0; it < ITEMS; it++) {
-            if (it * THREADS + wbase < cnt) {
-                const uint32_t idx = it * THREADS + tid;
-                const uint32_t s = sn[it] & 0xffffu, n = idx < cnt ? sn[it] >> 16 : 0u;
-                uint32_t rank = 0, eq = 0;
-                if (n > 1) {
-                    for (uint32_t j = 0; j < n; j++) {
-                        const uint64_t kj = keyS[s + j];
-                        rank += kj < key[it] ? 1u : 0u;
-                        eq += kj == key[it] ? 1u : 0u;
-                    }
-                    if (eq > 1) s_tie = 1u;
-                }
-                sn[it] = (s + rank) | (n << 16);
-            }
-        }
-        __syncthreads();
-        if (s_tie) {
-            // exact re-rank by (H, n): taken when two records of one bin carry the same 64-bit hash
+        uint32_t non[ITEMS], sn[ITEMS];                 // sn: slot, later position | bin size << 16
+        uint32_t cc[ITEMS];
+        uint32_t M = 0;
+        bool finished = false;
+        for (;;) {
+            for (int i = tid; i < (int)(VX_NBINS + 32) / 4; i += THREADS)
+                reinterpret_cast<uint4 *>(bins)[i] = make_uint4(0u, 0u, 0u, 0u);
+            __syncthreads();
+            if (tid == 0) s_tie = 0u;                   // set in phase E, read after the sync behind it
+            tile = s_tile;
+            if (tile >= q.P) { finished = true; break; }
+            cnt = min(q.cursor[tile], q.cap);
+            base1 = q.part_base[tile];
+            src = q.part + (size_t)tile * q.cap;
+
+            // ---- A. load + bin count -----------------------------------------------------------
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 const uint32_t idx = it * THREADS + tid;
-                if (idx < cnt) {
-                    const uint32_t b = (uint32_t)(key[it] >> binshift) & (VX_NBINS - 1);
-                    const uint32_t s = bins[b], e = bins[b + 1];
-                    uint32_t rank = 0;
-                    for (uint32_t j = s; j < e; j++) {
-                        const uint64_t kj = keyS[j];
-                        rank += (kj < key[it] || (kj == key[it] && nonS[j] < non[it])) ? 1u : 0u;
+                const uint4 r = idx < cnt ? __ldcs(src + idx) : make_uint4(0u, 0u, 0u, 0u);
+                key[it] = ((uint64_t)r.y << 32) | r.x;
+                non[it] = r.z;
+            }
+#pragma unroll
+            for (int it = 0; it < ITEMS; it++) {
+                const uint32_t idx = it * THREADS + tid;
+                if (idx < cnt) sn[it] = atomicAdd(&bins[(uint32_t)(key[it] >> binshift) & (VX_NBINS - 1)], 1u);
+            }
+            __syncthreads();
+            // ---- B. scan -------------------------------------------------------------------------
+            {
+                const uint32_t total = vx_block_exscan<THREADS, VX_NBINS / THREADS>(bins, s_warp);
+                if (tid == 0) bins[VX_NBINS] = total;
+            }
+            __syncthreads();
+            // ---- C. scatter to bin start + slot -----------------------------------------------------
+#pragma unroll
+            for (int it = 0; it < ITEMS; it++) {
+                if (it * THREADS + wbase < cnt) {       // warp-uniform
+                    const uint32_t idx = it * THREADS + tid;
+                    if (idx < cnt) {
+                        const uint32_t b = (uint32_t)(key[it] >> binshift) & (VX_NBINS - 1);
+                        const uint32_t s = bins[b], e = bins[b + 1];
+                        const uint32_t pos = s + sn[it];
+                        keyS[pos] = key[it];
+                        nonS[pos] = non[it];
+                        sn[it] = s | ((e - s) << 16);
+                    } else {
+                        sn[it] = 0u;
                     }
-                    sn[it] = (s + rank) | ((e - s) << 16);
+                }
+            }
+            if (tid == 0) keyS[cnt] = ~0ull;            // sentinel behind the last record
+            __syncthreads();
+            // ---- D. rank inside multi-record bins -----------------------------------------------------
+            if (!exact) {
+                // by H alone, warp lock-step over the largest bin of the warp's 32 records
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    if (it * THREADS + wbase < cnt) {
+                        const uint32_t s = sn[it] & 0xffffu;
+                        uint32_t n = sn[it] >> 16;
+                        if (n == 1) n = 0;              // alone in its bin: stays
+                        const uint32_t nm = __reduce_max_sync(VX_FULL, n);
+                        const uint64_t *kp = keyS + s;
+                        uint32_t rank = 0;
+                        for (uint32_t j = 0; j < nm; j++)
+                            if (j < n) rank += kp[j] < key[it] ? 1u : 0u;
+                        sn[it] = (s + rank) | (n << 16);
+                    }
+                }
+            } else {
+                // by (H, n), reading A10
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    const uint32_t idx = it * THREADS + tid;
+                    if (idx < cnt) {
+                        const uint32_t s = sn[it] & 0xffffu, n = sn[it] >> 16;
+                        uint32_t rank = 0;
+                        for (uint32_t j = s; j < s + n; j++) {
+                            const uint64_t kj = keyS[j];
+                            rank += (kj < key[it] || (kj == key[it] && nonS[j] < non[it])) ? 1u : 0u;
+                        }
+                        sn[it] = (s + rank) | ((n > 1 ? n : 0u) << 16);
+                    }
                 }
             }
             __syncthreads();
-        }
 #pragma unroll
-        for (int it = 0; it < ITEMS; it++) {
-            if (it * THREADS + wbase < cnt) {
-                const uint32_t idx = it * THREADS + tid;
-                if (idx < cnt && (sn[it] >> 16) > 1) {
-                    const uint32_t pos = sn[it] & 0xffffu;
-                    keyS[pos] = key[it];
-                    nonS[pos] = non[it];
+            for (int it = 0; it < ITEMS; it++) {
+                if (it * THREADS + wbase < cnt) {
+                    if (sn[it] >> 16) {
+                        const uint32_t pos = sn[it] & 0xffffu;
+                        keyS[pos] = key[it];
+                        nonS[pos] = non[it];
+                    }
                 }
             }
+            __syncthreads();
+            // ---- E. match count: lane i counts its successors within reach ----------------------
+            if (q.do_match) {
+                const uint32_t last = cnt ? cnt - 1 : 0u;
+                const bool guarded = tile == q.P - 1;   // only there can lim reach the sentinel
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    const uint32_t i = it * THREADS + tid;
+                    uint32_t c = 0;
+                    if (it * THREADS + wbase < cnt) {
+                        const uint64_t ki = keyS[min(i, cnt)];
+                        uint64_t lim = ki + Tm1;
+                        if (lim < ki) lim = ~0ull;
+                        lim = min(lim, ki | bmask);
+                        if (!guarded) {
+                            // the fast pass is valid iff the keys came out strictly increasing
+                            if (!exact && i < cnt && keyS[i + 1] <= ki) s_tie = 1u;
+                            // largest o in [0, 7] with key[i + o] <= lim (keys ascend; key[cnt] = ~0 > lim)
+                            uint32_t pos = i;
+                            if (keyS[min(pos + 4, cnt)] <= lim) pos += 4;
+                            if (keyS[min(pos + 2, cnt)] <= lim) pos += 2;
+                            if (keyS[min(pos + 1, cnt)] <= lim) pos += 1;
+                            c = i < cnt ? pos - i : 0u;
+                            if (__any_sync(VX_FULL, c == 7u)) {
+                                for (uint32_t j = i + 8;; j++) {
+                                    const bool m = c >= 7u && j < cnt && keyS[min(j, last)] <= lim;
+                                    c += m ? 1u : 0u;
+                                    if (!__any_sync(VX_FULL, m)) break;
+                                }
+                            }
+                        } else {
+                            if (!exact && i < last && keyS[i + 1] <= ki) s_tie = 1u;
+                            for (uint32_t j = i + 1;; j++) {
+                                const bool m = j < cnt && keyS[min(j, last)] <= lim;
+                                c += m ? 1u : 0u;
+                                if (!__any_sync(VX_FULL, m)) break;
+                            }
+                        }
+                    }
+                    cc[it] = c;
+                    E[i] = c;
+                }
+            }
+            __syncthreads();
+            if (!exact && s_tie) { exact = 1u; continue; }   // block-uniform: redo this tile exactly
+            break;
         }
-        __syncthreads();
+        if (finished) break;
 
         // first sorted position of local bucket bl (bl == 2^fb gives cnt)
         auto bucket_start = [&](uint32_t bl) -> uint32_t {
@@ -264,43 +320,17 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             return s;
         };
 
-        // ---- E. match count: lane i counts its successors within reach ------------------------------
-        uint32_t cc[ITEMS];
         unsigned long long base2 = 0;
-        uint32_t M = 0;
         if (q.do_match) {
-            const uint32_t last = cnt ? cnt - 1 : 0u;
-#pragma unroll
-            for (int it = 0; it < ITEMS; it++) {
-                const uint32_t i = it * THREADS + tid;
-                uint32_t c = 0;
-                if (it * THREADS + wbase < cnt) {
-                    const uint64_t ki = keyS[min(i, last)];
-                    uint64_t lim = ki + Tm1;
-                    if (lim < ki) lim = ~0ull;
-                    lim = min(lim, ki | bmask);
-                    uint32_t j = i + 1;
-                    for (;;) {
-                        const uint64_t k1 = keyS[min(j, last)], k2 = keyS[min(j + 1, last)];
-                        const bool m1 = j < cnt && k1 <= lim, m2 = j + 1 < cnt && k2 <= lim;
-                        c += (m1 ? 1u : 0u) + (m2 ? 1u : 0u);
-                        if (!__any_sync(VX_FULL, m2)) break;
-                        j += 2;
-                    }
-                }
-                cc[it] = c;
-                E[i] = c;
-            }
-            __syncthreads();
-            // ---- F. scan, publish the aggregate ---------------------------------------------------------
+            // ---- F. scan, publish the aggregate ---------------------------------------------------
             M = vx_block_exscan<THREADS, ITEMS>(E, s_warp);
             if (tid == 0) {
                 E[CAPA] = M;
                 if (tile) ((volatile unsigned long long *)q.status)[tile] = VX_ST_AGG | M;
             }
+            __syncthreads();
         }
-        __syncthreads();
-        // ---- G. sorted partition back in place; CSR offsets of Table 1 ---------------------------------
+        // ---- G. sorted partition back in place; CSR offsets of Table 1 ---------------------------
 #pragma unroll
         for (int it = 0; it < ITEMS; it++) {
             if (it * THREADS + wbase < cnt) {
@@ -321,14 +351,14 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         if (tile == q.P - 1 && tid == 0) q.t1_off[q.NB] = base1 + cnt;
 
         if (q.do_match) {
-            // ---- look-back for the Table-2 base ----------------------------------------------------------
+            // ---- look-back for the Table-2 base ----------------------------------------------------
             if (tid < 32) {
                 const unsigned long long b2 = vx_lookback(q.status, tile, M, lane);
                 if (tid == 0) s_base2 = b2;
             }
             __syncthreads();
             base2 = s_base2;
-            // ---- H. emit: the matches of i are i+1 .. i+c_i ------------------------------------------------
+            // ---- H. emit: the matches of i are i+1 .. i+c_i ------------------------------------------
             if (base2 + M > q.t2_cap) {
                 if (tid == 0) atomicOr(&q.ctrl->flags, VX_FLAG_T2_OVERFLOW);
             } else {
@@ -339,10 +369,14 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         const uint32_t c = cc[it];
                         const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
                         if (cmax) {
-                            const uint32_t ni = nonS[min(i, CAPA - 1)];
+                            const uint32_t ni = nonS[i];
+                            const uint32_t *np = nonS + i + 1;
                             uint2 *dst = q.t2_rec + (base2 + E[i]);
-                            for (uint32_t t = 0; t < cmax; t++)
-                                if (t < c) dst[t] = make_uint2(ni, nonS[i + 1 + t]);
+#pragma unroll
+                            for (uint32_t t = 0; t < 4; t++)
+                                if (t < c) dst[t] = make_uint2(ni, np[t]);
+                            for (uint32_t t = 4; t < cmax; t++)
+                                if (t < c) dst[t] = make_uint2(ni, np[t]);
                         }
                     }
                 }
@@ -400,7 +434,7 @@ cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, ui
 size_t vx_stage2_smem_bytes(const VxGeom &)
 {
     constexpr size_t CAPA = (size_t)VX_S2_THREADS * VX_S2_ITEMS;
-    return CAPA * 8 + CAPA * 4 + (VX_NBINS + 32) * 4 + (CAPA + 32) * 4;
+    return (CAPA + 2) * 8 + CAPA * 4 + (VX_NBINS + 32) * 4 + (CAPA + 32) * 4;
 }
 
 cudaError_t vx_stage2_configure(void)
