@@ -12,11 +12,22 @@
 // hash-prefix partitions of ~2^VX_TILE_LOG records each (they fit one CTA's shared memory);
 // stage 2 splits a partition into its 2^fb buckets (fb = B - pb) with a shared-memory
 // distribution sort over VX_BIN_BITS more hash bits (about one record per bin).
+#ifndef VX_TILE_LOG
 #define VX_TILE_LOG 12          // log2 of the mean records per partition
-#define VX_BIN_BITS 12          // bins per partition in stage 2 = 2^VX_BIN_BITS
+#endif
+#ifndef VX_BIN_BITS
+#define VX_BIN_BITS VX_TILE_LOG // bins per partition in stage 2 = 2^VX_BIN_BITS (one per record)
+#endif
 #define VX_NBINS (1u << VX_BIN_BITS)
+#ifndef VX_S2_THREADS
 #define VX_S2_THREADS 512
+#endif
+#ifndef VX_S2_ITEMS
 #define VX_S2_ITEMS 9           // VX_S2_THREADS * VX_S2_ITEMS >= max partition capacity
+#endif
+#ifndef VX_S2_MINB
+#define VX_S2_MINB 2            // resident CTAs per SM the fused kernel is compiled for
+#endif
 #define VX_MAX_CAP (VX_S2_THREADS * VX_S2_ITEMS)
 #define VX_STAGE_MAX_BYTES ((size_t)64 << 20) // Table-1 export staging (vx_read_tables)
 #define VX_MAX_MEAN_BUCKET_LOG 9 // K - B <= 9  (mean bucket <= 512 records, BASELINE.json K=33)

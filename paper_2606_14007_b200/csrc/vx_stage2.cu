@@ -112,7 +112,7 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
         unsigned long long s = VX_ST_INC;   // lanes before tile 0 count as "inclusive, value 0"
         if (idx >= 0) {
             s = vs[idx];
-            while ((s >> 62) == 0) { __nanosleep(100); s = vs[idx]; }
+            while ((s >> 62) == 0) { __nanosleep(200); s = vs[idx]; }
         }
         const unsigned incmask = __ballot_sync(VX_FULL, (s >> 62) == 2);
         unsigned long long v = s & VX_ST_VAL;
@@ -130,8 +130,14 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
     return excl;
 }
 
+// the 32 hash bits right below the bin index (bin = (H >> binshift) & (VX_NBINS - 1))
+__device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int binshift)
+{
+    return binshift >= 32 ? (uint32_t)(k >> (binshift - 32)) : (uint32_t)k << (32 - binshift);
+}
+
 template <int THREADS, int ITEMS>
-__global__ void __launch_bounds__(THREADS, 2)
+__global__ void __launch_bounds__(THREADS, VX_S2_MINB)
 vx_k_sort_match(const __grid_constant__ VxS2Params q)
 {
     constexpr int CAPA = THREADS * ITEMS;               // allocated sorted positions
@@ -140,6 +146,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     uint32_t *nonS = (uint32_t *)(keyS + CAPA + 2);     // CAPA sorted nonces (low 32 bits)
     uint32_t *bins = nonS + CAPA;                       // VX_NBINS + 1 (+ pad)
     uint32_t *E = bins + VX_NBINS + 32;                 // CAPA + 1 (+ pad): match-count prefix
+    uint32_t *sub = E;                                  // phases C-D only: 32-bit ranking sub-keys
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_tile, s_tie;
     __shared__ unsigned long long s_base2;
@@ -197,56 +204,63 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 if (tid == 0) bins[VX_NBINS] = total;
             }
             __syncthreads();
-            // ---- C. scatter to bin start + slot -----------------------------------------------------
+            // ---- C. scatter to bin start + slot (bank-random, the only such pass) ------------------
+            // sub[] = the 32 hash bits below the bin index: what the fast ranking pass compares
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 if (it * THREADS + wbase < cnt) {       // warp-uniform
                     const uint32_t idx = it * THREADS + tid;
                     if (idx < cnt) {
-                        const uint32_t b = (uint32_t)(key[it] >> binshift) & (VX_NBINS - 1);
-                        const uint32_t s = bins[b], e = bins[b + 1];
-                        const uint32_t pos = s + sn[it];
+                        const uint32_t pos = bins[(uint32_t)(key[it] >> binshift) & (VX_NBINS - 1)] + sn[it];
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
-                        sn[it] = s | ((e - s) << 16);
-                    } else {
-                        sn[it] = 0u;
+                        sub[pos] = vx_subkey(key[it], binshift);
                     }
                 }
             }
             if (tid == 0) keyS[cnt] = ~0ull;            // sentinel behind the last record
             __syncthreads();
-            // ---- D. rank inside multi-record bins -----------------------------------------------------
-            if (!exact) {
-                // by H alone, warp lock-step over the largest bin of the warp's 32 records
+            // ---- D. rank inside multi-record bins, one lane per position (neighbouring lanes
+            //         read neighbouring bins: conflict-free), warp lock-step over the largest bin -----
 #pragma unroll
-                for (int it = 0; it < ITEMS; it++) {
-                    if (it * THREADS + wbase < cnt) {
-                        const uint32_t s = sn[it] & 0xffffu;
-                        uint32_t n = sn[it] >> 16;
-                        if (n == 1) n = 0;              // alone in its bin: stays
-                        const uint32_t nm = __reduce_max_sync(VX_FULL, n);
-                        const uint64_t *kp = keyS + s;
-                        uint32_t rank = 0;
-                        for (uint32_t j = 0; j < nm; j++)
-                            if (j < n) rank += kp[j] < key[it] ? 1u : 0u;
-                        sn[it] = (s + rank) | (n << 16);
-                    }
-                }
-            } else {
-                // by (H, n), reading A10
+            for (int it = 0; it < ITEMS; it++) {
+                if (it * THREADS + wbase < cnt) {
+                    const uint32_t i = it * THREADS + tid;
+                    const uint64_t k = keyS[min(i, cnt)];
+                    const uint32_t nn = nonS[i];
+                    const uint32_t b = (uint32_t)(k >> binshift) & (VX_NBINS - 1);
+                    const uint32_t s = bins[b];
+                    uint32_t n = bins[b + 1] - s;
+                    if (i >= cnt || n == 1) n = 0;      // alone in its bin: stays
+                    const uint32_t nm = __reduce_max_sync(VX_FULL, n);
+                    uint32_t rank = 0;
+                    if (!exact) {
+                        // by the 32 bits below the bin index; equal sub-keys (or equal hashes) give
+                        // equal ranks, which phase E sees as keys that do not strictly increase
+                        const uint32_t *sp = sub + s;
+                        const uint32_t ks = vx_subkey(k, binshift);
 #pragma unroll
-                for (int it = 0; it < ITEMS; it++) {
-                    const uint32_t idx = it * THREADS + tid;
-                    if (idx < cnt) {
-                        const uint32_t s = sn[it] & 0xffffu, n = sn[it] >> 16;
-                        uint32_t rank = 0;
-                        for (uint32_t j = s; j < s + n; j++) {
-                            const uint64_t kj = keyS[j];
-                            rank += (kj < key[it] || (kj == key[it] && nonS[j] < non[it])) ? 1u : 0u;
+                        for (uint32_t j = 0; j < 4; j++) {
+                            const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
+                            rank += kj < ks ? 1u : 0u;
                         }
-                        sn[it] = (s + rank) | ((n > 1 ? n : 0u) << 16);
+                        if (nm > 4) {
+#pragma unroll 1
+                            for (uint32_t j = 4; j < nm; j++) {
+                                const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
+                                rank += kj < ks ? 1u : 0u;
+                            }
+                        }
+                    } else {                            // by (H, n), reading A10
+                        const uint64_t *kp = keyS + s;
+                        const uint32_t *np = nonS + s;
+#pragma unroll 1
+                        for (uint32_t j = 0; j < nm; j++)
+                            if (j < n) rank += (kp[j] < k || (kp[j] == k && np[j] < nn)) ? 1u : 0u;
                     }
+                    key[it] = k;
+                    non[it] = nn;
+                    sn[it] = (s + rank) | (n << 16);
                 }
             }
             __syncthreads();
@@ -468,7 +482,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
     const size_t smem = vx_stage2_smem_bytes(g);
-    uint64_t grid = (uint64_t)num_sms * 2;
+    uint64_t grid = (uint64_t)num_sms * VX_S2_MINB;
     if (grid > g.P) grid = g.P;
     vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS><<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
     return cudaGetLastError();
