@@ -53,7 +53,7 @@ typedef enum {
     VX_ERR_CUDA = -4,      /* a CUDA runtime call failed; text in vx_last_error                    */
     VX_ERR_OVERFLOW = -5,  /* a partition's slack or the Table-2 capacity overflowed on the device */
     VX_ERR_RANGE = -6,     /* bucket range outside [0, 2^B] or records_capacity too small          */
-    VX_ERR_UNSUPPORTED = -7 /* K valid per the paper's problem but not built yet (K > 32)          */
+    VX_ERR_UNSUPPORTED = -7 /* reserved: a valid configuration this build does not implement        */
 } vx_status;
 
 /* Device bytes the caller must provide for a plot of this K (B = 24 buckets bits, the paper's
@@ -62,11 +62,19 @@ size_t vx_workspace_bytes(uint32_t K);
 /* Same for a test-only bucket_bits (see vx_plot_create_ex). */
 size_t vx_workspace_bytes_ex(uint32_t K, uint32_t bucket_bits);
 
-/* Create a plot handle for 2^K nonces under a 256-bit key (host pointer, copied).  K in 1..32
- * (33..40 return VX_ERR_UNSUPPORTED until the 5-byte-nonce path lands).  PAPER.md L41-43. */
+/* Create a plot handle for 2^K nonces under a 256-bit key (host pointer, copied).  K in 1..33 with
+ * 2^24 buckets (mean bucket <= 512 records, BASELINE.json's K=33); K = 33 uses 5-byte nonces
+ * (reading A1) and the compact "wide" internal layout below.  PAPER.md L41-43. */
 vx_status vx_plot_create(uint32_t K, const uint8_t key[32], vx_plot **out);
 /* Test-only: bucket_bits B in 1..24 instead of 24 (dense buckets at tiny K, reading A7). */
 vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out);
+/* Test-only flags.  VX_CREATE_WIDE_LAYOUT: use the K >= 33 internal layout at this K, so that the
+ * wide kernels can be compared with the oracle on full small tables (results are identical by
+ * construction; the external formats do not change). */
+#define VX_CREATE_WIDE_LAYOUT 1u
+vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, uint32_t flags,
+                              vx_plot **out);
+size_t vx_workspace_bytes_opts(uint32_t K, uint32_t bucket_bits, uint32_t flags);
 
 /* Attach caller-owned device memory (>= vx_workspace_bytes, 256-byte aligned).  The workspace
  * holds Table 1 (the partition array), Table 2, their offsets, the look-back state and a small
@@ -108,7 +116,13 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
  *     dev_partition_base = uint64[2^pb + 1], the CSR index of each partition's first record:
  *     bucket b (partition q = b >> (B - pb)) starts at slot
  *     q * partition_capacity + dev_t1_offsets[b] - dev_partition_base[q].
- *   vx_read_tables converts to the external 12-byte Table-1 format on the way out. */
+ *   vx_read_tables converts to the external 12-byte Table-1 format on the way out.
+ *   Wide layout (K >= 33: a 16-byte record per nonce does not fit beside Table 2 in 180 GB): same
+ *     slot numbering, but dev_t1_records = uint64 a[2^pb * partition_capacity] with
+ *     a = (H << pb) | (n >> 12) -- the pb-bit hash prefix is the partition index, the bits it frees
+ *     hold the high nonce bits -- followed (vx_plot_info: layout) by uint16 b[] = n & 0xfff; sorting
+ *     by (a, b) is sorting by (H, n).  dev_t2_records = uint2 {n1 & 0xffffffff, n2 & 0xffffffff},
+ *     followed by uint8 hi[] = (n1 >> 32) | (n2 >> 32) << 4.  vx_read_tables converts both. */
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
                            const void **dev_t2_records, const uint64_t **dev_t2_offsets,
                            const uint64_t **dev_partition_base);

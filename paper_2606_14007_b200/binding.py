@@ -15,11 +15,13 @@ from . import build as _build
 
 VX_OK = 0
 VX_OPT_FORCE_EXACT_RANK = 1
+VX_CREATE_WIDE_LAYOUT = 1
 STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",
           -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED"}
 
 #: every symbol include/vx.h declares
-EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_plot_create", "vx_plot_create_ex",
+EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_opts", "vx_plot_create",
+           "vx_plot_create_ex", "vx_plot_create_opts",
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_read_tables",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink",
@@ -65,6 +67,10 @@ def load_library() -> ctypes.CDLL:
     L.vx_plot_create.argtypes = [_u32, ctypes.c_char_p, ctypes.POINTER(_vp)]
     L.vx_plot_create_ex.restype = ctypes.c_int
     L.vx_plot_create_ex.argtypes = [_u32, ctypes.c_char_p, _u32, ctypes.POINTER(_vp)]
+    L.vx_workspace_bytes_opts.restype = _sz
+    L.vx_workspace_bytes_opts.argtypes = [_u32, _u32, _u32]
+    L.vx_plot_create_opts.restype = ctypes.c_int
+    L.vx_plot_create_opts.argtypes = [_u32, ctypes.c_char_p, _u32, _u32, ctypes.POINTER(_vp)]
     L.vx_plot_bind.restype = ctypes.c_int
     L.vx_plot_bind.argtypes = [_vp, _vp, _sz]
     L.vx_build_table1.restype = ctypes.c_int
@@ -97,8 +103,8 @@ def load_library() -> ctypes.CDLL:
     return L
 
 
-def workspace_bytes(K: int, bucket_bits: int = 24) -> int:
-    return int(load_library().vx_workspace_bytes_ex(K, bucket_bits))
+def workspace_bytes(K: int, bucket_bits: int = 24, flags: int = 0) -> int:
+    return int(load_library().vx_workspace_bytes_opts(K, bucket_bits, flags))
 
 
 def _stream_ptr(stream) -> int:
@@ -111,15 +117,16 @@ def _stream_ptr(stream) -> int:
 class Plot:
     """One plot (K, key): vx_plot_create + vx_plot_bind on a torch-owned workspace."""
 
-    def __init__(self, K: int, key: bytes, bucket_bits: int = 24, device="cuda:0", workspace=None):
+    def __init__(self, K: int, key: bytes, bucket_bits: int = 24, device="cuda:0", workspace=None,
+                 flags: int = 0):
         import torch
         if len(key) != 32:
             raise ValueError("key must be 32 bytes")
         self._L = load_library()
         self._h = _vp()
-        st = self._L.vx_plot_create_ex(K, bytes(key), bucket_bits, ctypes.byref(self._h))
+        st = self._L.vx_plot_create_opts(K, bytes(key), bucket_bits, flags, ctypes.byref(self._h))
         if st != VX_OK:
-            raise VxError(st, f"vx_plot_create_ex(K={K}, bucket_bits={bucket_bits})")
+            raise VxError(st, f"vx_plot_create_opts(K={K}, bucket_bits={bucket_bits}, flags={flags})")
         self.K, self.bucket_bits = K, bucket_bits
         info = [_u32() for _ in range(5)]
         t2cap = _u64()
@@ -130,7 +137,7 @@ class Plot:
         self.t2_capacity = t2cap.value
         self.rec1_bytes = self.nonce_size + 8
         self.rec2_bytes = 2 * self.nonce_size
-        need = int(self._L.vx_workspace_bytes_ex(K, bucket_bits))
+        need = int(self._L.vx_workspace_bytes_opts(K, bucket_bits, flags))
         if not torch.cuda.is_available():
             self.free()
             raise VxError(-4, "no CUDA device: libvx has no CPU fallback")

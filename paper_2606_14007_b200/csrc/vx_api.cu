@@ -29,13 +29,14 @@ struct vx_plot {
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // ------------------------------------------------------------------------------ geometry
-bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B)
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide)
 {
     memset(g, 0, sizeof *g);
-    if (K < 1 || K > 40 || B < 1 || B > 24) return false;
+    if (K < 1 || K > 36 || B < 1 || B > 24) return false;  // wide Table-2 records keep 4 high nonce bits
     if (K > B + VX_MAX_MEAN_BUCKET_LOG) return false;
     g->K = K; g->B = B;
     g->nonce_size = K <= 32 ? 4 : 5;                       // reading A1
+    g->wide = (g->nonce_size > 4 || force_wide) ? 1u : 0u;
     g->pb = K > VX_TILE_LOG ? K - VX_TILE_LOG : 0;
     if (g->pb > B) return false;                           // cannot happen while K - B <= 9
     g->fb = B - g->pb;
@@ -56,10 +57,16 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B)
     g->off_cursor = o;    o = align256(o + g->P * 4);
     g->off_part_base = o; o = align256(o + (g->P + 1) * 8);
     g->off_status = o;    o = align256(o + g->P * 8);
-    g->off_part = o;      o = align256(o + g->P * (size_t)g->cap * 16);
+    if (!g->wide) {
+        g->off_part = o;  o = align256(o + g->P * (size_t)g->cap * 16);
+    } else {
+        g->off_part = o;   o = align256(o + g->P * (size_t)g->cap * 8);
+        g->off_part_b = o; o = align256(o + g->P * (size_t)g->cap * 2);
+    }
     g->off_t1_off = o;    o = align256(o + (g->NB + 1) * 8);
     g->off_t2_off = o;    o = align256(o + (g->NB + 1) * 8);
-    g->off_t2_rec = o;    o = align256(o + g->t2_cap * (size_t)g->rec2_bytes);
+    g->off_t2_rec = o;    o = align256(o + g->t2_cap * (size_t)8);
+    if (g->wide) { g->off_t2_hi = o; o = align256(o + g->t2_cap); }
     g->stage_bytes = g->N * (size_t)g->rec1_bytes;
     if (g->stage_bytes > VX_STAGE_MAX_BYTES) g->stage_bytes = VX_STAGE_MAX_BYTES;
     g->off_stage = o;     o = align256(o + g->stage_bytes);
@@ -144,23 +151,27 @@ const char *vx_status_string(vx_status s)
     return "VX_ERR_?";
 }
 
-size_t vx_workspace_bytes_ex(uint32_t K, uint32_t bucket_bits)
+size_t vx_workspace_bytes_opts(uint32_t K, uint32_t bucket_bits, uint32_t flags)
 {
     VxGeom g;
-    if (!vx_geom_init(&g, K, bucket_bits) || g.nonce_size != 4) return 0;
+    if (flags & ~(uint32_t)VX_CREATE_WIDE_LAYOUT) return 0;
+    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0)) return 0;
     return g.total;
 }
 
-size_t vx_workspace_bytes(uint32_t K) { return vx_workspace_bytes_ex(K, 24); }
+size_t vx_workspace_bytes_ex(uint32_t K, uint32_t bucket_bits) { return vx_workspace_bytes_opts(K, bucket_bits, 0); }
 
-vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out)
+size_t vx_workspace_bytes(uint32_t K) { return vx_workspace_bytes_opts(K, 24, 0); }
+
+vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, uint32_t flags,
+                              vx_plot **out)
 {
     if (!out) return VX_ERR_ARG;
     *out = NULL;
     if (!key) return VX_ERR_ARG;
+    if (flags & ~(uint32_t)VX_CREATE_WIDE_LAYOUT) return VX_ERR_ARG;
     VxGeom g;
-    if (!vx_geom_init(&g, K, bucket_bits)) return VX_ERR_ARG;
-    if (g.nonce_size != 4) return VX_ERR_UNSUPPORTED;
+    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0)) return VX_ERR_ARG;
     vx_plot *p = new (std::nothrow) vx_plot;
     if (!p) return VX_ERR_ARG;
     memset(p, 0, sizeof *p);
@@ -171,6 +182,11 @@ vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_b
     snprintf(p->err, sizeof p->err, "VX_OK");
     *out = p;
     return VX_OK;
+}
+
+vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out)
+{
+    return vx_plot_create_opts(K, key, bucket_bits, 0, out);
 }
 
 vx_status vx_plot_create(uint32_t K, const uint8_t key[32], vx_plot **out)
@@ -268,8 +284,22 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
     if (!records_out) return VX_OK;
     if (records_capacity < need) return fail(p, VX_ERR_RANGE, "records_capacity too small");
     if (need == 0) return VX_OK;
+    if (table == 2 && p->g.nonce_size > 4) {
+        // wide records (n1 lo, n2 lo) + high-bits byte -> external 10-byte records through staging
+        const uint64_t per2 = p->g.stage_bytes / rb;
+        for (uint64_t done = 0; done < last - first; done += per2) {
+            const uint64_t n = (last - first - done) < per2 ? (last - first - done) : per2;
+            e = vx_launch_export_t2(p->g, p->ws, first + done, n, p->stream);
+            if (e != cudaSuccess) return fail_cuda(p, e, "export launch");
+            e = cudaMemcpyAsync((uint8_t *)records_out + done * rb, p->ws + p->g.off_stage, n * rb,
+                                cudaMemcpyDeviceToHost, p->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+            if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(exported records)");
+        }
+        return VX_OK;
+    }
     if (table == 2) {
-        // Table 2 is resident in the external format: one contiguous copy
+        // Table 2 is resident in the external format (4-byte nonces): one contiguous copy
         e = cudaMemcpy(records_out, p->ws + p->g.off_t2_rec + (size_t)first * rb, need, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(records)");
         return VX_OK;

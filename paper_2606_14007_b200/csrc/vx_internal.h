@@ -34,6 +34,7 @@
 
 struct VxGeom {
     uint32_t K, B, nonce_size;
+    uint32_t wide; // compact 10-byte internal Table-1 records + 9-byte Table-2 records (K >= 33, or forced)
     uint32_t pb;   // partition bits: partition = H >> (64 - pb)
     uint32_t fb;   // bucket bits inside a partition, B - pb
     uint32_t cap;  // partition capacity in records (mean + slack, multiple of 32)
@@ -45,8 +46,12 @@ struct VxGeom {
     // workspace carve-up (byte offsets, each 256-aligned)
     size_t off_ctrl, off_cursor, off_part_base, off_status;
     size_t off_part;   // partition records: uint4 {H lo, H hi, nonce lo, nonce hi} per record;
-                       // after stage 2 each partition is sorted: this IS the resident Table 1
+                       // after stage 2 each partition is sorted: this IS the resident Table 1.
+                       // wide: uint64 a = (H << pb) | (n >> 12) per record (the partition prefix of H is
+                       // implied, the freed pb bits hold the high nonce bits) ...
+    size_t off_part_b; // ... wide only: uint16 b = n & 0xfff per record (same slot numbering)
     size_t off_t1_off, off_t2_off, off_t2_rec;
+    size_t off_t2_hi;  // wide only: uint8 per Table-2 record, (n1 >> 32) | (n2 >> 32) << 4
     size_t off_stage, stage_bytes;   // export staging for vx_read_tables(Table 1)
     size_t total;
 };
@@ -64,7 +69,7 @@ struct VxCtrl {
 #define VX_FLAG_T2_OVERFLOW 2u
 
 // returns false if (K, B) is not a supported geometry
-bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B);
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide);
 
 // host fold of the nonce-independent part of round 1 (vx_blake3.cuh)
 void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_size);
@@ -75,6 +80,8 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
                              cudaStream_t st);
 // external-format Table-1 records [first, first + count) of the CSR numbering -> ws + off_stage
 cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
+// wide, NONCE_SIZE = 5: external 10-byte Table-2 records [first, first + count) -> ws + off_stage
+cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
 cudaError_t vx_launch_hash_range(const VxGeom &g, const VxHashConst &hc, uint64_t nonce_begin,
                                  uint64_t count, uint64_t *dev_hashes, cudaStream_t st);
 cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t count,

@@ -28,6 +28,14 @@
 
 struct VxS2Params {
     uint4 *part;                 // partition records {H lo, H hi, nonce lo, nonce hi}; sorted in place
+                                 // (wide: uint64 a = (H << pb) | (n >> 12), with part_b: uint16 n & 0xfff)
+    uint16_t *part_b;
+    uint8_t *t2_hi;              // wide: (n1 >> 32) | (n2 >> 32) << 4 per Table-2 record
+    // sort key geometry (host-computed; the sort key is H, or a in the wide layout):
+    unsigned long long Tm1;      // (T - 1) in key units: (2^(64-K) - 1) << (wide ? pb : 0)
+    unsigned long long bmask;    // key | bmask = largest key of the key's bucket
+    unsigned long long lowmask;  // wide: the low pb key bits that hold nonce bits, else 0
+    int binshift, bshift;        // bin = (key >> binshift) & (NBINS-1); bucket-in-tile = (key >> bshift) & fbmask
     const uint32_t *cursor;
     const unsigned long long *part_base;
     unsigned long long *status;
@@ -136,7 +144,7 @@ __device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int binshift)
     return binshift >= 32 ? (uint32_t)(k >> (binshift - 32)) : (uint32_t)k << (32 - binshift);
 }
 
-template <int THREADS, int ITEMS>
+template <int THREADS, int ITEMS, bool WIDE>
 __global__ void __launch_bounds__(THREADS, VX_S2_MINB)
 vx_k_sort_match(const __grid_constant__ VxS2Params q)
 {
@@ -152,11 +160,11 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     __shared__ unsigned long long s_base2;
 
     const int tid = threadIdx.x, lane = tid & 31, wbase = tid & ~31;
-    const int binshift = 64 - (int)q.pb - VX_BIN_BITS;
-    const int bshift = 64 - (int)q.B;                   // bucket = H >> bshift
+    const int binshift = q.binshift;
+    const int bshift = q.bshift;
     const uint32_t fbmask = (1u << q.fb) - 1u;
-    const uint64_t Tm1 = (1ull << (64 - q.K)) - 1ull;   // T - 1
-    const uint64_t bmask = (1ull << bshift) - 1ull;     // H | bmask = last hash of H's bucket
+    const uint64_t Tm1 = q.Tm1;                         // T - 1 in key units
+    const uint64_t bmask = q.bmask;                     // key | bmask = last key of the key's bucket
     uint32_t cta_max_bucket = 0;
 
     for (;;) {
@@ -168,6 +176,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         uint32_t tile, cnt;
         unsigned long long base1;
         uint4 *src;
+        unsigned short *src_b = nullptr;
         uint64_t key[ITEMS];
         uint32_t non[ITEMS], sn[ITEMS];                 // sn: slot, later position | bin size << 16
         uint32_t cc[ITEMS];
@@ -182,15 +191,25 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             if (tile >= q.P) { finished = true; break; }
             cnt = min(q.cursor[tile], q.cap);
             base1 = q.part_base[tile];
-            src = q.part + (size_t)tile * q.cap;
+            if constexpr (WIDE) {
+                src = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned long long *>(q.part) + (size_t)tile * q.cap);
+                src_b = q.part_b + (size_t)tile * q.cap;
+            } else {
+                src = q.part + (size_t)tile * q.cap;
+            }
 
             // ---- A. load + bin count -----------------------------------------------------------
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 const uint32_t idx = it * THREADS + tid;
-                const uint4 r = idx < cnt ? __ldcs(src + idx) : make_uint4(0u, 0u, 0u, 0u);
-                key[it] = ((uint64_t)r.y << 32) | r.x;
-                non[it] = r.z;
+                if constexpr (WIDE) {
+                    key[it] = idx < cnt ? __ldcs(reinterpret_cast<const unsigned long long *>(src) + idx) : 0ull;
+                    non[it] = idx < cnt ? __ldcs(src_b + idx) : 0u;
+                } else {
+                    const uint4 r = idx < cnt ? __ldcs(src + idx) : make_uint4(0u, 0u, 0u, 0u);
+                    key[it] = ((uint64_t)r.y << 32) | r.x;
+                    non[it] = r.z;
+                }
             }
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
@@ -278,16 +297,20 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             // ---- E. match count: lane i counts its successors within reach ----------------------
             if (q.do_match) {
                 const uint32_t last = cnt ? cnt - 1 : 0u;
-                const bool guarded = tile == q.P - 1;   // only there can lim reach the sentinel
+                // guarded: lim can reach the sentinel value ~0 (narrow: only in the last tile; wide:
+                // only if the tile's largest key is ~0 itself, else lim is clamped below it)
+                const bool guarded = WIDE ? keyS[last] == ~0ull : tile == q.P - 1;
 #pragma unroll
                 for (int it = 0; it < ITEMS; it++) {
                     const uint32_t i = it * THREADS + tid;
                     uint32_t c = 0;
                     if (it * THREADS + wbase < cnt) {
                         const uint64_t ki = keyS[min(i, cnt)];
-                        uint64_t lim = ki + Tm1;
-                        if (lim < ki) lim = ~0ull;
+                        const uint64_t kl = WIDE ? (ki | q.lowmask) : ki;
+                        uint64_t lim = kl + Tm1;
+                        if (lim < kl) lim = ~0ull;
                         lim = min(lim, ki | bmask);
+                        if (WIDE && !guarded) lim = min(lim, (uint64_t)(~0ull - 1ull));
                         if (!guarded) {
                             // the fast pass is valid iff the keys came out strictly increasing
                             if (!exact && i < cnt && keyS[i + 1] <= ki) s_tie = 1u;
@@ -351,7 +374,12 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 const uint32_t idx = it * THREADS + tid;
                 if (idx < cnt) {
                     const uint64_t k = keyS[idx];
-                    src[idx] = make_uint4((uint32_t)k, (uint32_t)(k >> 32), nonS[idx], 0u);
+                    if constexpr (WIDE) {
+                        reinterpret_cast<unsigned long long *>(src)[idx] = k;
+                        src_b[idx] = (unsigned short)nonS[idx];
+                    } else {
+                        src[idx] = make_uint4((uint32_t)k, (uint32_t)(k >> 32), nonS[idx], 0u);
+                    }
                 }
             }
         }
@@ -383,14 +411,26 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         const uint32_t c = cc[it];
                         const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
                         if (cmax) {
-                            const uint32_t ni = nonS[i];
-                            const uint32_t *np = nonS + i + 1;
-                            uint2 *dst = q.t2_rec + (base2 + E[i]);
+                            if constexpr (WIDE) {
+                                // nonce = (low pb key bits) << 12 | the 12 bits kept beside the key
+                                const uint64_t ni = ((keyS[i] & q.lowmask) << 12) | nonS[i];
+                                const unsigned long long at = base2 + E[i];
+                                for (uint32_t t = 0; t < cmax; t++)
+                                    if (t < c) {
+                                        const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << 12) | nonS[i + 1 + t];
+                                        q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
+                                        q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
+                                    }
+                            } else {
+                                const uint32_t ni = nonS[i];
+                                const uint32_t *np = nonS + i + 1;
+                                uint2 *dst = q.t2_rec + (base2 + E[i]);
 #pragma unroll
-                            for (uint32_t t = 0; t < 4; t++)
-                                if (t < c) dst[t] = make_uint2(ni, np[t]);
-                            for (uint32_t t = 4; t < cmax; t++)
-                                if (t < c) dst[t] = make_uint2(ni, np[t]);
+                                for (uint32_t t = 0; t < 4; t++)
+                                    if (t < c) dst[t] = make_uint2(ni, np[t]);
+                                for (uint32_t t = 4; t < cmax; t++)
+                                    if (t < c) dst[t] = make_uint2(ni, np[t]);
+                            }
                         }
                     }
                 }
@@ -411,11 +451,12 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
 // ------------------------------------------------------------------------------ export
 // Table-1 records [first, first + count) of the CSR numbering, gathered from the partition array
-// into the external format nonce[4] LE || hash[8] (digest bytes, = H big-endian) in `out`.
+// into the external format nonce[NS] LE || hash[8] (digest bytes, = H big-endian) in `out`.
+template <bool WIDE, int NS>
 __global__ void __launch_bounds__(256)
-vx_k_export_t1(const uint4 *__restrict__ part, const unsigned long long *__restrict__ part_base,
-               uint32_t P, uint32_t cap, unsigned long long first, unsigned long long count,
-               uint32_t *__restrict__ out)
+vx_k_export_t1(const uint4 *__restrict__ part, const uint16_t *__restrict__ part_b,
+               const unsigned long long *__restrict__ part_base, uint32_t P, uint32_t cap, uint32_t pb,
+               unsigned long long first, unsigned long long count, uint8_t *__restrict__ out)
 {
     for (unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; r < count;
          r += (unsigned long long)gridDim.x * blockDim.x) {
@@ -426,10 +467,46 @@ vx_k_export_t1(const uint4 *__restrict__ part, const unsigned long long *__restr
             const uint32_t mid = (lo + hi) >> 1;
             if (part_base[mid] <= g) lo = mid; else hi = mid;
         }
-        const uint4 rec = part[(size_t)lo * cap + (g - part_base[lo])];
-        out[3 * r + 0] = rec.z;
-        out[3 * r + 1] = __byte_perm(rec.y, 0, 0x0123);
-        out[3 * r + 2] = __byte_perm(rec.x, 0, 0x0123);
+        const size_t slot = (size_t)lo * cap + (g - part_base[lo]);
+        unsigned long long H, n;
+        if constexpr (WIDE) {
+            const unsigned long long a = reinterpret_cast<const unsigned long long *>(part)[slot];
+            H = pb ? ((unsigned long long)lo << (64 - pb)) | (a >> pb) : a;
+            n = ((a & ((1ull << pb) - 1ull)) << 12) | part_b[slot];
+        } else {
+            const uint4 rec = part[slot];
+            H = ((unsigned long long)rec.y << 32) | rec.x;
+            n = rec.z;
+        }
+        if constexpr (NS == 4) {
+            uint32_t *o = reinterpret_cast<uint32_t *>(out) + 3 * r;
+            o[0] = (uint32_t)n;
+            o[1] = __byte_perm((uint32_t)(H >> 32), 0, 0x0123);
+            o[2] = __byte_perm((uint32_t)H, 0, 0x0123);
+        } else {
+            uint8_t *o = out + (size_t)(NS + 8) * r;
+#pragma unroll
+            for (int j = 0; j < NS; j++) o[j] = (uint8_t)(n >> (8 * j));
+#pragma unroll
+            for (int j = 0; j < 8; j++) o[NS + j] = (uint8_t)(H >> (8 * (7 - j)));
+        }
+    }
+}
+
+// wide Table-2 records [first, first + count) -> external nonce1[5] || nonce2[5], little-endian
+__global__ void __launch_bounds__(256)
+vx_k_export_t2(const uint2 *__restrict__ rec, const uint8_t *__restrict__ hi, unsigned long long first,
+               unsigned long long count, uint8_t *__restrict__ out)
+{
+    for (unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; r < count;
+         r += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint2 v = rec[first + r];
+        const uint8_t h = hi[first + r];
+        uint8_t *o = out + 10 * r;
+#pragma unroll
+        for (int j = 0; j < 4; j++) { o[j] = (uint8_t)(v.x >> (8 * j)); o[5 + j] = (uint8_t)(v.y >> (8 * j)); }
+        o[4] = h & 15u;
+        o[9] = h >> 4;
     }
 }
 
@@ -439,9 +516,27 @@ cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, ui
     if (count == 0) return cudaSuccess;
     uint64_t grid = (count + 255) / 256;
     if (grid > 148 * 16) grid = 148 * 16;
-    vx_k_export_t1<<<(unsigned)grid, 256, 0, st>>>(
-        (const uint4 *)(ws + g.off_part), (const unsigned long long *)(ws + g.off_part_base),
-        (uint32_t)g.P, g.cap, first, count, (uint32_t *)(ws + g.off_stage));
+    const uint4 *part = (const uint4 *)(ws + g.off_part);
+    const uint16_t *part_b = (const uint16_t *)(ws + g.off_part_b);
+    const unsigned long long *pbase = (const unsigned long long *)(ws + g.off_part_base);
+    uint8_t *out = ws + g.off_stage;
+    if (g.nonce_size == 5)
+        vx_k_export_t1<true, 5><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, first, count, out);
+    else if (g.wide)
+        vx_k_export_t1<true, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, first, count, out);
+    else
+        vx_k_export_t1<false, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, first, count, out);
+    return cudaGetLastError();
+}
+
+cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count,
+                                cudaStream_t st)
+{
+    if (count == 0) return cudaSuccess;
+    uint64_t grid = (count + 255) / 256;
+    if (grid > 148 * 16) grid = 148 * 16;
+    vx_k_export_t2<<<(unsigned)grid, 256, 0, st>>>((const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi,
+                                                   first, count, ws + g.off_stage);
     return cudaGetLastError();
 }
 
@@ -454,7 +549,10 @@ size_t vx_stage2_smem_bytes(const VxGeom &)
 cudaError_t vx_stage2_configure(void)
 {
     VxGeom g{};
-    return cudaFuncSetAttribute(vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS>,
+    cudaError_t e = cudaFuncSetAttribute(vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vx_stage2_smem_bytes(g));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, true>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vx_stage2_smem_bytes(g));
 }
 
@@ -481,9 +579,29 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
+    q.part_b = (uint16_t *)(ws + g.off_part_b);
+    q.t2_hi = ws + g.off_t2_hi;
+    // sort-key geometry.  narrow: key = H.  wide: key = a = (H << pb) | (n >> 12)
+    const unsigned long long T = 1ull << (64 - g.K);
+    if (g.wide) {
+        q.binshift = 64 - VX_BIN_BITS;
+        q.bshift = 64 - (int)g.fb;                      // only used when fb > VX_BIN_BITS (then < 64)
+        q.lowmask = (1ull << g.pb) - 1ull;
+        q.Tm1 = (T - 1ull) << g.pb;
+        q.bmask = g.fb ? (1ull << (64 - g.fb)) - 1ull : ~0ull;
+    } else {
+        q.binshift = 64 - (int)g.pb - VX_BIN_BITS;
+        q.bshift = 64 - (int)g.B;
+        q.lowmask = 0ull;
+        q.Tm1 = T - 1ull;
+        q.bmask = (1ull << q.bshift) - 1ull;
+    }
     const size_t smem = vx_stage2_smem_bytes(g);
     uint64_t grid = (uint64_t)num_sms * VX_S2_MINB;
     if (grid > g.P) grid = g.P;
-    vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS><<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
+    if (g.wide)
+        vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, true><<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
+    else
+        vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, false><<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
     return cudaGetLastError();
 }

@@ -36,6 +36,11 @@ def test_workspace_bytes_arithmetic():
     # + Table 2 (17.2 GB) + offsets
     assert 50e9 < vx.workspace_bytes(31) < 60e9
     assert vx.workspace_bytes(32) < 120e9
+    # K=33: wide layout, 10-byte Table-1 records in place (96.6 GB) + 9-byte Table-2 records (77.3 GB)
+    assert 170e9 < vx.workspace_bytes(33) < 178e9
+    # the test-only wide layout is smaller than the 16-byte-record layout at the same K
+    assert 0 < vx.workspace_bytes(20, 24, vx.VX_CREATE_WIDE_LAYOUT) < vx.workspace_bytes(20, 24)
+    assert vx.workspace_bytes(20, 24, 2) == 0              # unknown flag
     assert vx.workspace_bytes(16, 12) > 0 and vx.workspace_bytes(16, 4) == 0
 
 
@@ -49,7 +54,11 @@ def test_create_validates_arguments():
     assert L.vx_plot_create(20, key, None) == -1
     assert L.vx_plot_create_ex(16, key, 25, ctypes.byref(h)) == -1
     assert L.vx_plot_create_ex(16, key, 4, ctypes.byref(h)) == -1      # mean bucket > 512
-    assert L.vx_plot_create(33, key, ctypes.byref(h)) == -7            # 5-byte nonces: not built yet
+    assert L.vx_plot_create_opts(16, key, 12, 2, ctypes.byref(h)) == -1  # unknown flag
+    assert L.vx_plot_create(33, key, ctypes.byref(h)) == 0 and h.value   # 5-byte nonces, wide layout
+    ns = ctypes.c_uint32()
+    assert L.vx_plot_info(h, None, None, ctypes.byref(ns), None, None, None) == 0 and ns.value == 5
+    L.vx_free(h)
     assert L.vx_plot_create(20, key, ctypes.byref(h)) == 0 and h.value
     info = [ctypes.c_uint32() for _ in range(5)]
     t2 = ctypes.c_uint64()

@@ -26,13 +26,14 @@ def u64(t):
 
 
 # ------------------------------------------------------------------ hash kernel alone (a2-a4)
-@pytest.mark.parametrize("K,seed", [(20, 1), (27, 27), (31, 31), (32, 5)])
+@pytest.mark.parametrize("K,seed", [(20, 1), (27, 27), (31, 31), (32, 5), (33, 33)])
 def test_hash_range_vs_oracle(vx, K, seed):
     key = vx_inputs.key_from_seed(seed)
     N = 1 << K
-    for begin, count in ((0, 70001), (N - 4099, 4099), (N // 2 - 17, 1025)):
+    nsize = oracle.nonce_size(K)                 # 5-byte nonces from K = 33 (reading A1)
+    for begin, count in ((0, 70001), (N - 4099, 4099), (N // 2 - 17, 1025), (min(N, 1 << 32) - 600, 1200 if K > 32 else 600)):
         got = u64(vx.hash_range(K, key, begin, count))
-        want = oracle.hash_range(key, 4, begin, count)
+        want = oracle.hash_range(key, nsize, begin, count)
         assert np.array_equal(got, want)
 
 
@@ -53,15 +54,13 @@ def test_hash_worked_values(vx):
         if ln.startswith("#") or not ln.strip():
             continue
         K, seed, n, hx = ln.split()
-        if int(K) > 32:
-            continue
         got = u64(vx.hash_range(int(K), vx_inputs.key_from_seed(int(seed)), int(n), 1))
         assert f"{int(got[0]):016x}" == hx
 
 
 # ------------------------------------------------------------------ full tables, small K
-def run_plot(vx, K, key, B, force_exact=False):
-    plot = vx.Plot(K, key, B)
+def run_plot(vx, K, key, B, force_exact=False, flags=0):
+    plot = vx.Plot(K, key, B, flags=flags)
     if force_exact:
         plot.set_option(vx.VX_OPT_FORCE_EXACT_RANK, 1)
     plot.build_table1()
@@ -124,6 +123,32 @@ def test_exact_rerank_path_gives_the_same_tables(vx, K, B, seed):
     assert np.array_equal(off2, o_t2o)
     g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
     assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+
+
+WIDE_CASES = [(4, 2, 3), (10, 6, 2), (12, 8, 1), (12, 12, 7), (13, 8, 4), (16, 12, 1), (16, 7, 6),
+              (18, 24, 3), (20, 24, 1), (21, 12, 2), (22, 24, 22)]
+
+
+@pytest.mark.parametrize("force_exact", [False, True])
+@pytest.mark.parametrize("K,B,seed", WIDE_CASES)
+def test_wide_layout_gives_the_same_tables(vx, K, B, seed, force_exact):
+    """The K >= 33 internal layout (10-byte Table-1 records a = (H << pb) | (n >> 12), b = n & 0xfff;
+    Table-2 records with a high-bits byte), forced at small K: bit-exact against the oracle."""
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    (off_b, raw_b), (off1, raw1), (off2, raw2), stats, nsize = run_plot(
+        vx, K, key, B, force_exact=force_exact, flags=vx.VX_CREATE_WIDE_LAYOUT)
+    assert nsize == 4
+    assert np.array_equal(off_b, o_off)
+    nb, hb = canon_t1(off_b, *decode_t1(raw_b, nsize))
+    assert np.array_equal(nb, o_non) and np.array_equal(hb, o_has)
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(nsize, o_non, o_has))
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    sizes = np.diff(o_off)
+    assert stats == {"t1_records": 1 << K, "t2_records": len(o_n1), "max_bucket": int(sizes.max())}
 
 
 def test_device_tables_layout(vx):
