@@ -188,3 +188,83 @@ def test_K31_full_size_samples_and_properties(vx):
     stats = whole_table_properties(plot, K)
     assert stats["t1_records"] == 1 << 31
     plot.free()
+
+
+def wide_views(plot):
+    """Device views of the wide layout (include/vx.h, vx_device_tables): a[], b[], part_base, offsets."""
+    import torch
+    t1, t1o, t2, t2o, pbase = plot.device_tables()
+    ws, base = plot.workspace, plot.workspace.data_ptr()
+    P, cap, NB = 1 << plot.partition_bits, plot.partition_capacity, 1 << plot.bucket_bits
+    a_off = t1 - base
+    b_off = (a_off + P * cap * 8 + 255) & ~255
+    a = ws[a_off: a_off + P * cap * 8].view(torch.int64).view(P, cap)
+    b = ws[b_off: b_off + P * cap * 2].view(torch.int16).view(P, cap)
+    pb = ws[pbase - base: pbase - base + (P + 1) * 8].view(torch.int64)
+    o1 = ws[t1o - base: t1o - base + (NB + 1) * 8].view(torch.int64)
+    o2 = ws[t2o - base: t2o - base + (NB + 1) * 8].view(torch.int64)
+    return a, b, pb, o1, o2
+
+
+def test_K33_full_size_samples_and_properties(vx):
+    """BASELINE.json configs[4]: 2^33 nonces, 5-byte nonces, ~512 records per bucket, 174 GB of
+    tables on one B200.  Sampled buckets hash by hash against the oracle (5-byte keyed hash) with
+    their Table 2 bit-exact; whole-table properties on the device: every nonce exactly once, every
+    partition sorted by (H, n), CSR offsets consistent, |T2| within 6 sigma of the closed form."""
+    import torch
+    K, B = 33, 24
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    need = vx.workspace_bytes(K)
+    if free < need + (6 << 30):
+        pytest.skip(f"needs {need / 1e9:.0f} GB + 6 GB of device memory, {free / 1e9:.0f} GB free")
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    assert plot.nonce_size == 5
+    plot.build_table1()
+    plot.sort_match_table2()
+    stats = plot.get_stats()
+    N = 1 << K
+    assert stats["t1_records"] == N
+    mean = N * (1 - 2.0 ** (B - K - 1))
+    assert abs(stats["t2_records"] - mean) < 6 * mean ** 0.5 + 8
+    rng = np.random.default_rng(33)
+    starts = [0, (1 << 24) - 4] + [int(x) for x in rng.integers(0, (1 << 24) - 4, 14)]
+    n = check_sampled_buckets(plot, K, key, [(s, s + 4) for s in starts])
+    assert n > 25000
+
+    a, b, pb, o1, o2 = wide_views(plot)
+    dev = plot.device
+    pbits, cap = plot.partition_bits, plot.partition_capacity
+    P = 1 << pbits
+    cnt = pb[1:] - pb[:-1]
+    assert int(pb[0]) == 0 and int(pb[-1]) == N and int(cnt.max()) <= cap
+    assert int(o1[0]) == 0 and int(o1[-1]) == N and bool((o1[1:] >= o1[:-1]).all())
+    assert stats["max_bucket"] == int((o1[1:] - o1[:-1]).max())
+    assert int(o2[0]) == 0 and int(o2[-1]) == stats["t2_records"] and bool((o2[1:] >= o2[:-1]).all())
+    # bucket b of partition q starts at slot offsets[b] - part_base[q]: bucket sizes sum to the partition
+    fb = B - pbits
+    assert bool((o1[:-1][:: 1 << fb] == pb[:-1]).all())
+    lane = torch.arange(cap, device=dev)[None, :]
+    chunk = (1 << 25) // cap
+    lowmask = (1 << pbits) - 1
+    R = 1 << 30                                          # nonce range checked per pass
+    for r0 in range(0, N, R):
+        seen = torch.zeros(R, dtype=torch.bool, device=dev)
+        for p0 in range(0, P, chunk):
+            ak = a[p0:p0 + chunk]
+            valid = lane < cnt[p0:p0 + chunk, None]
+            bk = b[p0:p0 + chunk].long() & 0xffff
+            if r0 == 0:
+                assert bool((bk[valid] < 4096).all())
+                k = ak ^ SIGN                            # unsigned order of a through a signed compare
+                ok = (k[:, 1:] > k[:, :-1]) | ((k[:, 1:] == k[:, :-1]) & (bk[:, 1:] > bk[:, :-1]))
+                assert bool((ok | ~valid[:, 1:]).all()), "a partition is not sorted by (H, n)"
+                del k, ok
+            non = ((ak & lowmask) << 12) | bk
+            sel = valid & (non >= r0) & (non < r0 + R)
+            seen[non[sel] - r0] = True
+            del ak, valid, bk, non, sel
+        assert int(seen.sum()) == R, "some nonce is missing from Table 1 (or appears twice)"
+        del seen
+    plot.free()
