@@ -40,6 +40,10 @@ BUCKET_BITS = 24
 ALU_OPS_PER_NONCE = 415            # xor / rotate / byte-swap lane-ops that need the ALU pipe
 S2_BYTES_PER_NONCE = 12 + 12 + 8   # read record, write sorted record, write ~1 Table-2 record
 S1_BYTES_PER_NONCE = 12            # write the record once
+# DRAM bytes per nonce measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one
+# launch at K=29 / 2^29; profiles/r01_v3.md) -- the same kernels and tile geometry at every K
+S1_DRAM_BYTES_PER_NONCE_NCU = 21.8
+S2_DRAM_BYTES_PER_NONCE_NCU = 40.4
 
 
 def measured_peaks():
@@ -105,6 +109,27 @@ class ClockSampler:
         busy = [x for x in sm if x >= 0.5 * max(sm)] or sm
         return {"sm_mhz": statistics.median(busy), "sm_max_mhz": max(mx), "samples": len(sm),
                 "reasons": sorted(reasons)}
+
+
+def rank_seed(K: int, rank: int) -> int:
+    """Independent plots: rank r plots under key SplitMix64(seed_for_K + 1000 r)."""
+    import vx_inputs
+    return vx_inputs.seed_for_K(K) + 1000 * rank
+
+
+def max_over_ranks(values, world: int, device=None):
+    """Element-wise MAX over ranks of a list of floats (times are max-over-ranks, never summed)."""
+    import torch
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.tolist()]
+
+
+def whole_job_value(K: int, world: int, ms_per_step: float) -> float:
+    """nonces/s over all ranks: every rank makes one whole plot per step (weak scaling)."""
+    return world * (1 << K) / (ms_per_step * 1e-3)
 
 
 def make_config(K: int):
@@ -192,7 +217,7 @@ def run_cuda(args):
 
     K = args.K
     # independent plots: rank r plots under key SplitMix64(seed_for_K + 1000 r)
-    key = vx_inputs.key_from_seed(vx_inputs.seed_for_K(K) + 1000 * rank)
+    key = vx_inputs.key_from_seed(rank_seed(K, rank))
     plot = vx.Plot(K, key, BUCKET_BITS, device=dev)
     N = 1 << K
     stream = torch.cuda.current_stream()
@@ -256,28 +281,27 @@ def run_cuda(args):
     e2e_s = (time.perf_counter() - t0) / e2e_steps
 
     # ---- max over ranks -------------------------------------------------------------------
-    vals = torch.tensor([total_ms, e2e_s, statistics.mean(s1_ms), statistics.mean(s2_ms)],
-                        dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
-    total_ms, e2e_s, s1, s2 = [float(x) for x in vals.tolist()]
+    total_ms, e2e_s, s1, s2 = max_over_ranks(
+        [total_ms, e2e_s, statistics.mean(s1_ms), statistics.mean(s2_ms)], world, dev)
     ms_per_step = total_ms / args.steps
 
     if rank == 0:
         peaks = measured_peaks()
         alu_peak = 148 * 4 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12     # T lane-ops/s on the ALU pipe
         r1 = {"kernel": "vx_k_hash_scatter", "bound": "alu", "achieved": ALU_OPS_PER_NONCE * N / (s1 * 1e-3) / 1e12,
-              "peak": alu_peak, "unit": "Tlaneop/s", "traffic": None, "ms": s1,
+              "peak": alu_peak, "unit": "Tlaneop/s", "traffic": S1_DRAM_BYTES_PER_NONCE_NCU * N, "ms": s1,
               "hbm_algorithmic_GBps": S1_BYTES_PER_NONCE * N / (s1 * 1e-3) / 1e9}
         r1["frac"] = r1["achieved"] / r1["peak"]
         r2 = {"kernel": "vx_k_sort_match", "bound": "hbm", "achieved": S2_BYTES_PER_NONCE * N / (s2 * 1e-3) / 1e9,
-              "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": None, "ms": s2}
+              "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": S2_DRAM_BYTES_PER_NONCE_NCU * N, "ms": s2}
         r2["frac"] = r2["achieved"] / r2["peak"]
         dominant = dict(r1 if s1 >= s2 else r2)
+        dominant["traffic_source"] = ("ncu --set full at K=29 (profiles/r01_v3.md): DRAM read+write bytes per "
+                                      "nonce of this kernel x 2^K")
         dominant["peak_source"] = peaks["source"] + (" (hbm_gbs, burst copy)" if dominant["bound"] == "hbm"
                                                      else " (sm_max_mhz x 148 SM x 4 SMSP x 16 ALU lanes; DESIGN.md)")
         line = {
-            "metric": METRIC, "value": world * N / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "metric": METRIC, "value": whole_job_value(K, world, ms_per_step), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64",
             "data": "synthetic",
@@ -286,7 +310,7 @@ def run_cuda(args):
             "stages": {"build_table1": {"ms": s1, "nonces_per_s": N / (s1 * 1e-3), "roofline": r1},
                        "sort_match_table2": {"ms": s2, "nonces_per_s": N / (s2 * 1e-3), "roofline": r2}},
             "table_stats": stats,
-            "roofline": {k: dominant[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel", "peak_source")},
+            "roofline": {k: dominant[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel", "peak_source", "traffic_source")},
             "e2e": {"value": world * N / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 32,
                     "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
                     "what": "vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2 + vx_read_tables(Table 2, "
