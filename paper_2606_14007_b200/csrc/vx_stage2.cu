@@ -120,7 +120,7 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
         unsigned long long s = VX_ST_INC;   // lanes before tile 0 count as "inclusive, value 0"
         if (idx >= 0) {
             s = vs[idx];
-            while ((s >> 62) == 0) { __nanosleep(200); s = vs[idx]; }
+            for (unsigned ns = 128; (s >> 62) == 0; ns = min(ns * 2u, 1024u)) { __nanosleep(ns); s = vs[idx]; }
         }
         const unsigned incmask = __ballot_sync(VX_FULL, (s >> 62) == 2);
         unsigned long long v = s & VX_ST_VAL;
@@ -139,9 +139,15 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
 }
 
 // the 32 hash bits right below the bin index (bin = (H >> binshift) & (VX_NBINS - 1))
-__device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int binshift)
+// binshift >= 32 always (pb + VX_BIN_BITS <= 32; checked at launch), so both are 32-bit operations on
+// the high word: sh = binshift - 32
+__device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int sh)
 {
-    return binshift >= 32 ? (uint32_t)(k >> (binshift - 32)) : (uint32_t)k << (32 - binshift);
+    return __funnelshift_r((uint32_t)k, (uint32_t)(k >> 32), sh);
+}
+__device__ __forceinline__ uint32_t vx_bin(uint64_t k, int sh)
+{
+    return ((uint32_t)(k >> 32) >> sh) & (VX_NBINS - 1);
 }
 
 template <int THREADS, int ITEMS, bool WIDE>
@@ -151,7 +157,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     constexpr int CAPA = THREADS * ITEMS;               // allocated sorted positions
     extern __shared__ __align__(16) uint8_t vx_smem[];
     uint64_t *keyS = (uint64_t *)vx_smem;               // CAPA sorted hashes + sentinel (+ pad)
-    uint32_t *nonS = (uint32_t *)(keyS + CAPA + 2);     // CAPA sorted nonces (low 32 bits)
+    uint32_t *nonS = (uint32_t *)(keyS + CAPA + 8);     // CAPA sorted nonces (low 32 bits)
     uint32_t *bins = nonS + CAPA;                       // VX_NBINS + 1 (+ pad)
     uint32_t *E = bins + VX_NBINS + 32;                 // CAPA + 1 (+ pad): match-count prefix
     uint32_t *sub = E;                                  // phases C-D only: 32-bit ranking sub-keys
@@ -160,7 +166,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     __shared__ unsigned long long s_base2;
 
     const int tid = threadIdx.x, lane = tid & 31, wbase = tid & ~31;
-    const int binshift = q.binshift;
+    const int sh = q.binshift - 32;                     // bin / sub-key shifts act on the high key word
     const int bshift = q.bshift;
     const uint32_t fbmask = (1u << q.fb) - 1u;
     const uint64_t Tm1 = q.Tm1;                         // T - 1 in key units
@@ -214,7 +220,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 const uint32_t idx = it * THREADS + tid;
-                if (idx < cnt) sn[it] = atomicAdd(&bins[(uint32_t)(key[it] >> binshift) & (VX_NBINS - 1)], 1u);
+                if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin(key[it], sh)], 1u);
             }
             __syncthreads();
             // ---- B. scan -------------------------------------------------------------------------
@@ -230,14 +236,14 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 if (it * THREADS + wbase < cnt) {       // warp-uniform
                     const uint32_t idx = it * THREADS + tid;
                     if (idx < cnt) {
-                        const uint32_t pos = bins[(uint32_t)(key[it] >> binshift) & (VX_NBINS - 1)] + sn[it];
+                        const uint32_t pos = bins[vx_bin(key[it], sh)] + sn[it];
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
-                        sub[pos] = vx_subkey(key[it], binshift);
+                        sub[pos] = vx_subkey(key[it], sh);
                     }
                 }
             }
-            if (tid == 0) keyS[cnt] = ~0ull;            // sentinel behind the last record
+            if (tid < 8) keyS[cnt + tid] = ~0ull;       // sentinels behind the last record: no clamps in E
             __syncthreads();
             // ---- D. rank inside multi-record bins, one lane per position (neighbouring lanes
             //         read neighbouring bins: conflict-free), warp lock-step over the largest bin -----
@@ -245,9 +251,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             for (int it = 0; it < ITEMS; it++) {
                 if (it * THREADS + wbase < cnt) {
                     const uint32_t i = it * THREADS + tid;
-                    const uint64_t k = keyS[min(i, cnt)];
+                    const uint64_t k = keyS[i];         // i >= cnt: sentinel or stale, result unused
                     const uint32_t nn = nonS[i];
-                    const uint32_t b = (uint32_t)(k >> binshift) & (VX_NBINS - 1);
+                    const uint32_t b = vx_bin(k, sh);
                     const uint32_t s = bins[b];
                     uint32_t n = bins[b + 1] - s;
                     if (i >= cnt || n == 1) n = 0;      // alone in its bin: stays
@@ -257,7 +263,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         // by the 32 bits below the bin index; equal sub-keys (or equal hashes) give
                         // equal ranks, which phase E sees as keys that do not strictly increase
                         const uint32_t *sp = sub + s;
-                        const uint32_t ks = vx_subkey(k, binshift);
+                        const uint32_t ks = vx_subkey(k, sh);
 #pragma unroll
                         for (uint32_t j = 0; j < 4; j++) {
                             const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
@@ -305,10 +311,11 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t i = it * THREADS + tid;
                     uint32_t c = 0;
                     if (it * THREADS + wbase < cnt) {
-                        const uint64_t ki = keyS[min(i, cnt)];
+                        const uint64_t ki = keyS[i];
                         const uint64_t kl = WIDE ? (ki | q.lowmask) : ki;
                         uint64_t lim = kl + Tm1;
-                        if (lim < kl) lim = ~0ull;
+                        // narrow, not the last tile: key + T stays inside the next partition, no wrap
+                        if ((WIDE || guarded) && lim < kl) lim = ~0ull;
                         lim = min(lim, ki | bmask);
                         if (WIDE && !guarded) lim = min(lim, (uint64_t)(~0ull - 1ull));
                         if (!guarded) {
@@ -316,9 +323,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             if (!exact && i < cnt && keyS[i + 1] <= ki) s_tie = 1u;
                             // largest o in [0, 7] with key[i + o] <= lim (keys ascend; key[cnt] = ~0 > lim)
                             uint32_t pos = i;
-                            if (keyS[min(pos + 4, cnt)] <= lim) pos += 4;
-                            if (keyS[min(pos + 2, cnt)] <= lim) pos += 2;
-                            if (keyS[min(pos + 1, cnt)] <= lim) pos += 1;
+                            if (keyS[pos + 4] <= lim) pos += 4;
+                            if (keyS[pos + 2] <= lim) pos += 2;
+                            if (keyS[pos + 1] <= lim) pos += 1;
                             c = i < cnt ? pos - i : 0u;
                             if (__any_sync(VX_FULL, c == 7u)) {
                                 for (uint32_t j = i + 8;; j++) {
@@ -543,7 +550,7 @@ cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, ui
 size_t vx_stage2_smem_bytes(const VxGeom &)
 {
     constexpr size_t CAPA = (size_t)VX_S2_THREADS * VX_S2_ITEMS;
-    return (CAPA + 2) * 8 + CAPA * 4 + (VX_NBINS + 32) * 4 + (CAPA + 32) * 4;
+    return (CAPA + 8) * 8 + CAPA * 4 + (VX_NBINS + 32) * 4 + (CAPA + 32) * 4;
 }
 
 cudaError_t vx_stage2_configure(void)
@@ -579,6 +586,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
+    if (g.pb + VX_BIN_BITS > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
     q.part_b = (uint16_t *)(ws + g.off_part_b);
     q.t2_hi = ws + g.off_t2_hi;
     // sort-key geometry.  narrow: key = H.  wide: key = a = (H << pb) | (n >> 12)
