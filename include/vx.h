@@ -72,6 +72,9 @@ vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_b
  * wide kernels can be compared with the oracle on full small tables (results are identical by
  * construction; the external formats do not change). */
 #define VX_CREATE_WIDE_LAYOUT 1u
+/* VX_CREATE_BIG_TILES: use the K >= 32 tile geometry (2^13-record partitions, one 1024-thread CTA
+ * per SM) at this K, for the same reason. */
+#define VX_CREATE_BIG_TILES 2u
 vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, uint32_t flags,
                               vx_plot **out);
 size_t vx_workspace_bytes_opts(uint32_t K, uint32_t bucket_bits, uint32_t flags);
@@ -119,8 +122,8 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
  *   vx_read_tables converts to the external 12-byte Table-1 format on the way out.
  *   Wide layout (K >= 33: a 16-byte record per nonce does not fit beside Table 2 in 180 GB): same
  *     slot numbering, but dev_t1_records = uint64 a[2^pb * partition_capacity] with
- *     a = (H << pb) | (n >> 12) -- the pb-bit hash prefix is the partition index, the bits it frees
- *     hold the high nonce bits -- followed (vx_plot_info: layout) by uint16 b[] = n & 0xfff; sorting
+ *     a = (H << pb) | (n >> t) -- the pb-bit hash prefix is the partition index, the bits it frees
+ *     hold the high nonce bits -- followed (256-byte aligned) by uint16 b[] = n & (2^t - 1), t = vx_plot_layout's tile_log; sorting
  *     by (a, b) is sorting by (H, n).  dev_t2_records = uint2 {n1 & 0xffffffff, n2 & 0xffffffff},
  *     followed by uint8 hi[] = (n1 >> 32) | (n2 >> 32) << 4.  vx_read_tables converts both. */
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
@@ -152,6 +155,10 @@ vx_status vx_hash_sink(vx_plot *p, uint64_t count, uint64_t *dev_sink, size_t si
 /* Plot geometry, for tests and the bench report.  Any pointer may be NULL. */
 vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uint32_t *nonce_size,
                        uint32_t *partition_bits, uint32_t *partition_capacity, uint64_t *t2_capacity);
+
+/* Internal layout, for callers of vx_device_tables: wide = 1 for the 10-byte Table-1 layout;
+ * tile_log = log2 of the mean partition size (12 for K <= 31, 13 from K = 32). */
+vx_status vx_plot_layout(const vx_plot *p, uint32_t *wide, uint32_t *tile_log);
 
 const char *vx_last_error(const vx_plot *p); /* never NULL; includes cudaGetErrorString text */
 const char *vx_status_string(vx_status s);

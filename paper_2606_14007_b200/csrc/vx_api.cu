@@ -29,7 +29,7 @@ struct vx_plot {
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // ------------------------------------------------------------------------------ geometry
-bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide)
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles)
 {
     memset(g, 0, sizeof *g);
     if (K < 1 || K > 36 || B < 1 || B > 24) return false;  // wide Table-2 records keep 4 high nonce bits
@@ -37,7 +37,8 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide)
     g->K = K; g->B = B;
     g->nonce_size = K <= 32 ? 4 : 5;                       // reading A1
     g->wide = (g->nonce_size > 4 || force_wide) ? 1u : 0u;
-    g->pb = K > VX_TILE_LOG ? K - VX_TILE_LOG : 0;
+    g->tile_log = (K >= VX_BIG_TILES_FROM_K || force_big_tiles) ? VX_TILE_LOG_BIG : VX_TILE_LOG;
+    g->pb = K > g->tile_log ? K - g->tile_log : 0;
     if (g->pb > B) return false;                           // cannot happen while K - B <= 9
     g->fb = B - g->pb;
     g->N = 1ull << K; g->P = 1ull << g->pb; g->NB = 1ull << B;
@@ -46,7 +47,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide)
     if (g->pb == 0) cap = mean;                            // the single partition holds everything
     else cap = mean + (uint64_t)ceil(8.0 * sqrt((double)mean));        // Poisson tail, 8 sigma
     cap = (cap + 31) & ~(uint64_t)31;
-    if (cap > VX_MAX_CAP) return false;
+    if (cap > (g->tile_log == VX_TILE_LOG_BIG ? VX_S2B_THREADS * VX_S2B_ITEMS : VX_S2_THREADS * VX_S2_ITEMS)) return false;
     g->cap = (uint32_t)cap;
     // |T2| ~ 2^K (1 - 2^(B-K-1)) for K >= B, 2^(2K-1-B) below; sd ~ sqrt: 2^K + slack is ample
     g->t2_cap = g->N + (1u << 16);
@@ -154,8 +155,8 @@ const char *vx_status_string(vx_status s)
 size_t vx_workspace_bytes_opts(uint32_t K, uint32_t bucket_bits, uint32_t flags)
 {
     VxGeom g;
-    if (flags & ~(uint32_t)VX_CREATE_WIDE_LAYOUT) return 0;
-    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0)) return 0;
+    if (flags & ~(uint32_t)(VX_CREATE_WIDE_LAYOUT | VX_CREATE_BIG_TILES)) return 0;
+    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0, (flags & VX_CREATE_BIG_TILES) != 0)) return 0;
     return g.total;
 }
 
@@ -169,9 +170,9 @@ vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket
     if (!out) return VX_ERR_ARG;
     *out = NULL;
     if (!key) return VX_ERR_ARG;
-    if (flags & ~(uint32_t)VX_CREATE_WIDE_LAYOUT) return VX_ERR_ARG;
+    if (flags & ~(uint32_t)(VX_CREATE_WIDE_LAYOUT | VX_CREATE_BIG_TILES)) return VX_ERR_ARG;
     VxGeom g;
-    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0)) return VX_ERR_ARG;
+    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0, (flags & VX_CREATE_BIG_TILES) != 0)) return VX_ERR_ARG;
     vx_plot *p = new (std::nothrow) vx_plot;
     if (!p) return VX_ERR_ARG;
     memset(p, 0, sizeof *p);
@@ -387,6 +388,14 @@ vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uin
     if (partition_bits) *partition_bits = p->g.pb;
     if (partition_capacity) *partition_capacity = p->g.cap;
     if (t2_capacity) *t2_capacity = p->g.t2_cap;
+    return VX_OK;
+}
+
+vx_status vx_plot_layout(const vx_plot *p, uint32_t *wide, uint32_t *tile_log)
+{
+    if (!p) return VX_ERR_ARG;
+    if (wide) *wide = p->g.wide;
+    if (tile_log) *tile_log = p->g.tile_log;
     return VX_OK;
 }
 

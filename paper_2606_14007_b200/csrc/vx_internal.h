@@ -12,29 +12,23 @@
 // hash-prefix partitions of ~2^VX_TILE_LOG records each (they fit one CTA's shared memory);
 // stage 2 splits a partition into its 2^fb buckets (fb = B - pb) with a shared-memory
 // distribution sort over VX_BIN_BITS more hash bits (about one record per bin).
-#ifndef VX_TILE_LOG
-#define VX_TILE_LOG 12          // log2 of the mean records per partition
-#endif
-#ifndef VX_BIN_BITS
-#define VX_BIN_BITS VX_TILE_LOG // bins per partition in stage 2 = 2^VX_BIN_BITS (one per record)
-#endif
-#define VX_NBINS (1u << VX_BIN_BITS)
-#ifndef VX_S2_THREADS
+#define VX_TILE_LOG 12          // log2 of the mean records per partition, K <= 31
 #define VX_S2_THREADS 512
-#endif
-#ifndef VX_S2_ITEMS
-#define VX_S2_ITEMS 9           // VX_S2_THREADS * VX_S2_ITEMS >= max partition capacity
-#endif
-#ifndef VX_S2_MINB
+#define VX_S2_ITEMS 9           // VX_S2_THREADS * VX_S2_ITEMS >= partition capacity (mean + 8 sigma)
 #define VX_S2_MINB 2            // resident CTAs per SM the fused kernel is compiled for
-#endif
-#define VX_MAX_CAP (VX_S2_THREADS * VX_S2_ITEMS)
+// K >= 32: 2^(K-12) open partitions no longer stay resident in L2 during stage 1 (K=32 stage 1 was
+// 139 ms instead of 2 x 54); tiles of 2^13 records halve their number.  One 1024-thread CTA per SM.
+#define VX_TILE_LOG_BIG 13
+#define VX_S2B_THREADS 1024
+#define VX_S2B_ITEMS 9
+#define VX_BIG_TILES_FROM_K 32
 #define VX_STAGE_MAX_BYTES ((size_t)64 << 20) // Table-1 export staging (vx_read_tables)
 #define VX_MAX_MEAN_BUCKET_LOG 9 // K - B <= 9  (mean bucket <= 512 records, BASELINE.json K=33)
 
 struct VxGeom {
     uint32_t K, B, nonce_size;
     uint32_t wide; // compact 10-byte internal Table-1 records + 9-byte Table-2 records (K >= 33, or forced)
+    uint32_t tile_log; // log2 of the mean partition size: VX_TILE_LOG or VX_TILE_LOG_BIG
     uint32_t pb;   // partition bits: partition = H >> (64 - pb)
     uint32_t fb;   // bucket bits inside a partition, B - pb
     uint32_t cap;  // partition capacity in records (mean + slack, multiple of 32)
@@ -47,9 +41,9 @@ struct VxGeom {
     size_t off_ctrl, off_cursor, off_part_base, off_status;
     size_t off_part;   // partition records: uint4 {H lo, H hi, nonce lo, nonce hi} per record;
                        // after stage 2 each partition is sorted: this IS the resident Table 1.
-                       // wide: uint64 a = (H << pb) | (n >> 12) per record (the partition prefix of H is
+                       // wide: uint64 a = (H << pb) | (n >> tile_log) per record (the partition prefix of H is
                        // implied, the freed pb bits hold the high nonce bits) ...
-    size_t off_part_b; // ... wide only: uint16 b = n & 0xfff per record (same slot numbering)
+    size_t off_part_b; // ... wide only: uint16 b = n & (2^tile_log - 1) per record (same slot numbering)
     size_t off_t1_off, off_t2_off, off_t2_rec;
     size_t off_t2_hi;  // wide only: uint8 per Table-2 record, (n1 >> 32) | (n2 >> 32) << 4
     size_t off_stage, stage_bytes;   // export staging for vx_read_tables(Table 1)
@@ -69,7 +63,7 @@ struct VxCtrl {
 #define VX_FLAG_T2_OVERFLOW 2u
 
 // returns false if (K, B) is not a supported geometry
-bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide);
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles);
 
 // host fold of the nonce-independent part of round 1 (vx_blake3.cuh)
 void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_size);

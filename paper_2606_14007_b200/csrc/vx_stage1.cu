@@ -18,11 +18,11 @@
 #define VX_S1_NPT 4
 
 // WIDE (K >= 33, or forced by a test): the record is 10 bytes in two arrays with the same slot
-// numbering, a = (H << pb) | (n >> 12) (the partition prefix of H is implied by the partition, the
-// pb bits it frees hold the high nonce bits) and b = n & 0xfff -- DESIGN.md "wide layout".
+// numbering, a = (H << pb) | (n >> tile_log) (the partition prefix of H is implied by the partition, the
+// pb bits it frees hold the high nonce bits) and b = n & (2^tile_log - 1) -- DESIGN.md "wide layout".
 template <bool NONCE5, bool WIDE>
 __global__ void __launch_bounds__(VX_S1_THREADS)
-vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t pb, uint32_t cap,
+vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t pb, uint32_t nlo_bits, uint32_t cap,
                   uint4 *__restrict__ part, uint16_t *__restrict__ part_b,
                   uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
 {
@@ -41,8 +41,8 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t p
             const uint32_t slot = atomicAdd(&cursor[p], 1u);
             if (slot < cap) {
                 if constexpr (WIDE) {
-                    reinterpret_cast<uint64_t *>(part)[(uint64_t)p * cap + slot] = (H[k] << pb) | (n >> 12);
-                    part_b[(uint64_t)p * cap + slot] = (uint16_t)(n & 0xfffu);
+                    reinterpret_cast<uint64_t *>(part)[(uint64_t)p * cap + slot] = (H[k] << pb) | (n >> nlo_bits);
+                    part_b[(uint64_t)p * cap + slot] = (uint16_t)(n & ((1u << nlo_bits) - 1u));
                 } else {
                     // one 16-byte store per record: scattered stores are bound by requests, not bytes
                     part[(uint64_t)p * cap + slot] =
@@ -162,11 +162,11 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
     uint4 *part = (uint4 *)(ws + g.off_part);
     uint16_t *part_b = (uint16_t *)(ws + g.off_part_b);
     if (g.nonce_size == 5)
-        vx_k_hash_scatter<true, true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, part, part_b, cursor, ctrl);
+        vx_k_hash_scatter<true, true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.tile_log, g.cap, part, part_b, cursor, ctrl);
     else if (g.wide)
-        vx_k_hash_scatter<false, true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, part, part_b, cursor, ctrl);
+        vx_k_hash_scatter<false, true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.tile_log, g.cap, part, part_b, cursor, ctrl);
     else
-        vx_k_hash_scatter<false, false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.cap, part, part_b, cursor, ctrl);
+        vx_k_hash_scatter<false, false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.tile_log, g.cap, part, part_b, cursor, ctrl);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap, g.P,

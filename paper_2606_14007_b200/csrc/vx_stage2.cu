@@ -35,6 +35,7 @@ struct VxS2Params {
     unsigned long long Tm1;      // (T - 1) in key units: (2^(64-K) - 1) << (wide ? pb : 0)
     unsigned long long bmask;    // key | bmask = largest key of the key's bucket
     unsigned long long lowmask;  // wide: the low pb key bits that hold nonce bits, else 0
+    uint32_t nlo_bits;           // wide: nonce bits kept in part_b (= tile_log)
     int binshift, bshift;        // bin = (key >> binshift) & (NBINS-1); bucket-in-tile = (key >> bshift) & fbmask
     const uint32_t *cursor;
     const unsigned long long *part_base;
@@ -145,15 +146,21 @@ __device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int sh)
 {
     return __funnelshift_r((uint32_t)k, (uint32_t)(k >> 32), sh);
 }
+template <uint32_t NBINS>
 __device__ __forceinline__ uint32_t vx_bin(uint64_t k, int sh)
 {
-    return ((uint32_t)(k >> 32) >> sh) & (VX_NBINS - 1);
+    return ((uint32_t)(k >> 32) >> sh) & (NBINS - 1);
 }
 
-template <int THREADS, int ITEMS, bool WIDE>
-__global__ void __launch_bounds__(THREADS, VX_S2_MINB)
+// Two tile geometries are built (vx_internal.h): 2^12-record tiles, 512 threads, 2 CTAs per SM
+// (K <= 31) and 2^13-record tiles, 1024 threads, 1 CTA per SM (K >= 32, where stage 1 cannot keep
+// 2^(K-12) open partitions resident in L2).  BIN_BITS = log2 of the tile size: one bin per record.
+template <int THREADS, int ITEMS, int BIN_BITS, int MINB, bool WIDE>
+__global__ void __launch_bounds__(THREADS, MINB)
 vx_k_sort_match(const __grid_constant__ VxS2Params q)
 {
+    constexpr uint32_t VX_NBINS = 1u << BIN_BITS;       // (shadows nothing: the macros are gone)
+    constexpr int VX_BIN_BITS = BIN_BITS;
     constexpr int CAPA = THREADS * ITEMS;               // allocated sorted positions
     extern __shared__ __align__(16) uint8_t vx_smem[];
     uint64_t *keyS = (uint64_t *)vx_smem;               // CAPA sorted hashes + sentinel (+ pad)
@@ -220,7 +227,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 const uint32_t idx = it * THREADS + tid;
-                if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin(key[it], sh)], 1u);
+                if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin<VX_NBINS>(key[it], sh)], 1u);
             }
             __syncthreads();
             // ---- B. scan -------------------------------------------------------------------------
@@ -236,7 +243,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 if (it * THREADS + wbase < cnt) {       // warp-uniform
                     const uint32_t idx = it * THREADS + tid;
                     if (idx < cnt) {
-                        const uint32_t pos = bins[vx_bin(key[it], sh)] + sn[it];
+                        const uint32_t pos = bins[vx_bin<VX_NBINS>(key[it], sh)] + sn[it];
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
                         sub[pos] = vx_subkey(key[it], sh);
@@ -253,7 +260,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t i = it * THREADS + tid;
                     const uint64_t k = keyS[i];         // i >= cnt: sentinel or stale, result unused
                     const uint32_t nn = nonS[i];
-                    const uint32_t b = vx_bin(k, sh);
+                    const uint32_t b = vx_bin<VX_NBINS>(k, sh);
                     const uint32_t s = bins[b];
                     uint32_t n = bins[b + 1] - s;
                     if (i >= cnt || n == 1) n = 0;      // alone in its bin: stays
@@ -419,12 +426,12 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
                         if (cmax) {
                             if constexpr (WIDE) {
-                                // nonce = (low pb key bits) << 12 | the 12 bits kept beside the key
-                                const uint64_t ni = ((keyS[i] & q.lowmask) << 12) | nonS[i];
+                                // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key
+                                const uint64_t ni = ((keyS[i] & q.lowmask) << q.nlo_bits) | nonS[i];
                                 const unsigned long long at = base2 + E[i];
                                 for (uint32_t t = 0; t < cmax; t++)
                                     if (t < c) {
-                                        const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << 12) | nonS[i + 1 + t];
+                                        const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << q.nlo_bits) | nonS[i + 1 + t];
                                         q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
                                         q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
                                     }
@@ -463,6 +470,7 @@ template <bool WIDE, int NS>
 __global__ void __launch_bounds__(256)
 vx_k_export_t1(const uint4 *__restrict__ part, const uint16_t *__restrict__ part_b,
                const unsigned long long *__restrict__ part_base, uint32_t P, uint32_t cap, uint32_t pb,
+               uint32_t nlo_bits,
                unsigned long long first, unsigned long long count, uint8_t *__restrict__ out)
 {
     for (unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; r < count;
@@ -479,7 +487,7 @@ vx_k_export_t1(const uint4 *__restrict__ part, const uint16_t *__restrict__ part
         if constexpr (WIDE) {
             const unsigned long long a = reinterpret_cast<const unsigned long long *>(part)[slot];
             H = pb ? ((unsigned long long)lo << (64 - pb)) | (a >> pb) : a;
-            n = ((a & ((1ull << pb) - 1ull)) << 12) | part_b[slot];
+            n = ((a & ((1ull << pb) - 1ull)) << nlo_bits) | part_b[slot];
         } else {
             const uint4 rec = part[slot];
             H = ((unsigned long long)rec.y << 32) | rec.x;
@@ -528,11 +536,11 @@ cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, ui
     const unsigned long long *pbase = (const unsigned long long *)(ws + g.off_part_base);
     uint8_t *out = ws + g.off_stage;
     if (g.nonce_size == 5)
-        vx_k_export_t1<true, 5><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, first, count, out);
+        vx_k_export_t1<true, 5><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, g.tile_log, first, count, out);
     else if (g.wide)
-        vx_k_export_t1<true, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, first, count, out);
+        vx_k_export_t1<true, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, g.tile_log, first, count, out);
     else
-        vx_k_export_t1<false, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, first, count, out);
+        vx_k_export_t1<false, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, g.tile_log, first, count, out);
     return cudaGetLastError();
 }
 
@@ -547,20 +555,29 @@ cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, ui
     return cudaGetLastError();
 }
 
-size_t vx_stage2_smem_bytes(const VxGeom &)
+size_t vx_stage2_smem_bytes(const VxGeom &g)
 {
-    constexpr size_t CAPA = (size_t)VX_S2_THREADS * VX_S2_ITEMS;
-    return (CAPA + 8) * 8 + CAPA * 4 + (VX_NBINS + 32) * 4 + (CAPA + 32) * 4;
+    const size_t CAPA = g.tile_log == VX_TILE_LOG_BIG ? (size_t)VX_S2B_THREADS * VX_S2B_ITEMS
+                                                      : (size_t)VX_S2_THREADS * VX_S2_ITEMS;
+    const size_t nbins = (size_t)1 << g.tile_log;
+    return (CAPA + 8) * 8 + CAPA * 4 + (nbins + 32) * 4 + (CAPA + 32) * 4;
 }
+
+#define VX_S2_KERNEL(WIDE) vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, VX_TILE_LOG, VX_S2_MINB, WIDE>
+#define VX_S2B_KERNEL(WIDE) vx_k_sort_match<VX_S2B_THREADS, VX_S2B_ITEMS, VX_TILE_LOG_BIG, 1, WIDE>
 
 cudaError_t vx_stage2_configure(void)
 {
     VxGeom g{};
-    cudaError_t e = cudaFuncSetAttribute(vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vx_stage2_smem_bytes(g));
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, true>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vx_stage2_smem_bytes(g));
+    g.tile_log = VX_TILE_LOG;
+    const int small = (int)vx_stage2_smem_bytes(g);
+    g.tile_log = VX_TILE_LOG_BIG;
+    const int big = (int)vx_stage2_smem_bytes(g);
+    cudaError_t e = cudaFuncSetAttribute(VX_S2_KERNEL(false), cudaFuncAttributeMaxDynamicSharedMemorySize, small);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, small);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(false), cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    return e;
 }
 
 cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool force_exact, int num_sms,
@@ -586,30 +603,32 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
-    if (g.pb + VX_BIN_BITS > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
+    if (g.pb + g.tile_log > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
     q.part_b = (uint16_t *)(ws + g.off_part_b);
     q.t2_hi = ws + g.off_t2_hi;
     // sort-key geometry.  narrow: key = H.  wide: key = a = (H << pb) | (n >> 12)
     const unsigned long long T = 1ull << (64 - g.K);
     if (g.wide) {
-        q.binshift = 64 - VX_BIN_BITS;
+        q.binshift = 64 - (int)g.tile_log;
         q.bshift = 64 - (int)g.fb;                      // only used when fb > VX_BIN_BITS (then < 64)
         q.lowmask = (1ull << g.pb) - 1ull;
         q.Tm1 = (T - 1ull) << g.pb;
         q.bmask = g.fb ? (1ull << (64 - g.fb)) - 1ull : ~0ull;
     } else {
-        q.binshift = 64 - (int)g.pb - VX_BIN_BITS;
+        q.binshift = 64 - (int)g.pb - (int)g.tile_log;
         q.bshift = 64 - (int)g.B;
         q.lowmask = 0ull;
         q.Tm1 = T - 1ull;
         q.bmask = (1ull << q.bshift) - 1ull;
     }
     const size_t smem = vx_stage2_smem_bytes(g);
-    uint64_t grid = (uint64_t)num_sms * VX_S2_MINB;
+    q.nlo_bits = g.tile_log;
+    const bool big = g.tile_log == VX_TILE_LOG_BIG;
+    uint64_t grid = (uint64_t)num_sms * (big ? 1 : VX_S2_MINB);
     if (grid > g.P) grid = g.P;
-    if (g.wide)
-        vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, true><<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
-    else
-        vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, false><<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
+    if (big && g.wide) VX_S2B_KERNEL(true)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
+    else if (big) VX_S2B_KERNEL(false)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
+    else if (g.wide) VX_S2_KERNEL(true)<<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
+    else VX_S2_KERNEL(false)<<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
     return cudaGetLastError();
 }

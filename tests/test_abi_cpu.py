@@ -40,7 +40,8 @@ def test_workspace_bytes_arithmetic():
     assert 170e9 < vx.workspace_bytes(33) < 178e9
     # the test-only wide layout is smaller than the 16-byte-record layout at the same K
     assert 0 < vx.workspace_bytes(20, 24, vx.VX_CREATE_WIDE_LAYOUT) < vx.workspace_bytes(20, 24)
-    assert vx.workspace_bytes(20, 24, 2) == 0              # unknown flag
+    assert 0 < vx.workspace_bytes(20, 24, vx.VX_CREATE_BIG_TILES)
+    assert vx.workspace_bytes(20, 24, 4) == 0              # unknown flag
     assert vx.workspace_bytes(16, 12) > 0 and vx.workspace_bytes(16, 4) == 0
 
 
@@ -54,7 +55,7 @@ def test_create_validates_arguments():
     assert L.vx_plot_create(20, key, None) == -1
     assert L.vx_plot_create_ex(16, key, 25, ctypes.byref(h)) == -1
     assert L.vx_plot_create_ex(16, key, 4, ctypes.byref(h)) == -1      # mean bucket > 512
-    assert L.vx_plot_create_opts(16, key, 12, 2, ctypes.byref(h)) == -1  # unknown flag
+    assert L.vx_plot_create_opts(16, key, 12, 4, ctypes.byref(h)) == -1  # unknown flag
     assert L.vx_plot_create(33, key, ctypes.byref(h)) == 0 and h.value   # 5-byte nonces, wide layout
     ns = ctypes.c_uint32()
     assert L.vx_plot_info(h, None, None, ctypes.byref(ns), None, None, None) == 0 and ns.value == 5

@@ -256,12 +256,12 @@ def test_K33_full_size_samples_and_properties(vx):
             valid = lane < cnt[p0:p0 + chunk, None]
             bk = b[p0:p0 + chunk].long() & 0xffff
             if r0 == 0:
-                assert bool((bk[valid] < 4096).all())
+                assert bool((bk[valid] < (1 << plot.tile_log)).all())
                 k = ak ^ SIGN                            # unsigned order of a through a signed compare
                 ok = (k[:, 1:] > k[:, :-1]) | ((k[:, 1:] == k[:, :-1]) & (bk[:, 1:] > bk[:, :-1]))
                 assert bool((ok | ~valid[:, 1:]).all()), "a partition is not sorted by (H, n)"
                 del k, ok
-            non = ((ak & lowmask) << 12) | bk
+            non = ((ak & lowmask) << plot.tile_log) | bk
             sel = valid & (non >= r0) & (non < r0 + R)
             seen[non[sel] - r0] = True
             del ak, valid, bk, non, sel

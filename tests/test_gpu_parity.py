@@ -129,6 +129,27 @@ WIDE_CASES = [(4, 2, 3), (10, 6, 2), (12, 8, 1), (12, 12, 7), (13, 8, 4), (16, 1
               (18, 24, 3), (20, 24, 1), (21, 12, 2), (22, 24, 22)]
 
 
+@pytest.mark.parametrize("K,B,seed", [(10, 6, 2), (13, 8, 4), (14, 9, 5), (16, 12, 1), (16, 7, 6), (18, 24, 3),
+                                      (20, 24, 1), (21, 12, 2), (22, 24, 22)])
+@pytest.mark.parametrize("wide", [False, True])
+def test_big_tile_geometry_gives_the_same_tables(vx, K, B, seed, wide):
+    """The K >= 32 geometry (2^13-record partitions, one 1024-thread CTA per SM), forced at small K,
+    in both record layouts: bit-exact against the oracle."""
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    flags = vx.VX_CREATE_BIG_TILES | (vx.VX_CREATE_WIDE_LAYOUT if wide else 0)
+    (off_b, raw_b), (off1, raw1), (off2, raw2), stats, nsize = run_plot(vx, K, key, B, flags=flags)
+    assert np.array_equal(off_b, o_off)
+    nb, hb = canon_t1(off_b, *decode_t1(raw_b, nsize))
+    assert np.array_equal(nb, o_non) and np.array_equal(hb, o_has)
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(nsize, o_non, o_has))
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    assert stats["t2_records"] == len(o_n1)
+
+
 @pytest.mark.parametrize("force_exact", [False, True])
 @pytest.mark.parametrize("K,B,seed", WIDE_CASES)
 def test_wide_layout_gives_the_same_tables(vx, K, B, seed, force_exact):
