@@ -175,6 +175,31 @@ def test_K27_full_size_digests_and_samples(vx):
     plot.free()
 
 
+@pytest.mark.parametrize("K", [29, 32])
+def test_K29_K32_full_size_samples_and_properties(vx, K):
+    """BASELINE.json configs[2] (K=29, ~32 records per bucket) and K=32 (the first K on 2^13-record
+    tiles / 1024-thread CTAs), same checks as K=31."""
+    import torch
+    B = 24
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    need = vx.workspace_bytes(K) + (40 << 30 if K == 32 else 8 << 30)   # + the 2^K x 8 B hash stream
+    if free < need:
+        pytest.skip(f"needs {need / 1e9:.0f} GB of device memory, {free / 1e9:.0f} GB free")
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    assert plot.tile_log == (13 if K >= 32 else 12)
+    plot.build_table1()
+    plot.sort_match_table2()
+    rng = np.random.default_rng(K)
+    starts = [0, (1 << 24) - 8] + [int(x) for x in rng.integers(0, (1 << 24) - 8, 14)]
+    n = check_sampled_buckets(plot, K, key, [(s, s + 8) for s in starts])
+    assert n > 3000
+    stats = whole_table_properties(plot, K)
+    assert stats["t1_records"] == 1 << K
+    plot.free()
+
+
 def test_K31_full_size_samples_and_properties(vx):
     K, B = 31, 24
     key = vx_inputs.config_key(K)
