@@ -315,7 +315,7 @@ def run_cuda(args):
                     "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
                     "what": "vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2 + vx_read_tables(Table 2, "
                             f"{chunks} bucket ranges) into pinned host memory"},
-            "gpu_launches": 3 * args.steps,
+            "gpu_launches": plot.launches_per_plot * args.steps,
             "clocks": clocks,
         }
         if world == 1 and not args.no_cpu_baseline:

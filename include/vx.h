@@ -88,7 +88,10 @@ vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes);
  * into its hash-prefix partition in HBM.  Enqueues only.  After it, Table 1 is resident in HBM as
  * 2^P coarse hash-prefix buckets (P = max(K-12, 0) capped at B); the split of each coarse bucket
  * into its 2^(B-P) buckets is an in-shared-memory counting step of the fused kernel below (or
- * of vx_read_tables when Table 1 is read before vx_sort_match_table2).  See DESIGN.md "hierarchy". */
+ * of vx_read_tables when Table 1 is read before vx_sort_match_table2).  See DESIGN.md "hierarchy".
+ * Wide layout (K >= 33): the nonce space is hashed in 4 rounds; each round scatters its records,
+ * 16 bytes each, into scratch partitions that alias the (still unused) Table-2 region and then
+ * compacts them into the 10-byte partition array. */
 vx_status vx_build_table1(vx_plot *p, void *cuda_stream);
 
 /* Stage 2 (rows a6-a8; "fused ... single GPU kernel"): for every bucket, stage it in
@@ -159,6 +162,11 @@ vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uin
 /* Internal layout, for callers of vx_device_tables: wide = 1 for the 10-byte Table-1 layout;
  * tile_log = log2 of the mean partition size (12 for K <= 31, 13 from K = 32). */
 vx_status vx_plot_layout(const vx_plot *p, uint32_t *wide, uint32_t *tile_log);
+
+/* Kernels one vx_build_table1 / vx_sort_match_table2 call launches (for the bench report's
+ * gpu_launches): 2 + 1 in the narrow layout; the wide layout builds Table 1 in 4 rounds of
+ * hash+scatter and compaction: 2 * 4 + 1 launches. */
+vx_status vx_plot_launches(const vx_plot *p, uint32_t *build_table1, uint32_t *sort_match_table2);
 
 const char *vx_last_error(const vx_plot *p); /* never NULL; includes cudaGetErrorString text */
 const char *vx_status_string(vx_status s);

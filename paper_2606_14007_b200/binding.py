@@ -26,7 +26,7 @@ EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_op
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_read_tables",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink",
-           "vx_plot_info", "vx_plot_layout", "vx_last_error", "vx_status_string", "vx_free"]
+           "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
 
 _u64 = ctypes.c_uint64
 _u32 = ctypes.c_uint32
@@ -96,6 +96,8 @@ def load_library() -> ctypes.CDLL:
     L.vx_plot_info.argtypes = [_vp] + [ctypes.POINTER(_u32)] * 5 + [ctypes.POINTER(_u64)]
     L.vx_plot_layout.restype = ctypes.c_int
     L.vx_plot_layout.argtypes = [_vp, ctypes.POINTER(_u32), ctypes.POINTER(_u32)]
+    L.vx_plot_launches.restype = ctypes.c_int
+    L.vx_plot_launches.argtypes = [_vp, ctypes.POINTER(_u32), ctypes.POINTER(_u32)]
     L.vx_last_error.restype = ctypes.c_char_p
     L.vx_last_error.argtypes = [_vp]
     L.vx_status_string.restype = ctypes.c_char_p
@@ -141,6 +143,9 @@ class Plot:
         wide, tlog = _u32(), _u32()
         self._L.vx_plot_layout(self._h, ctypes.byref(wide), ctypes.byref(tlog))
         self.wide, self.tile_log = bool(wide.value), tlog.value
+        l1, l2 = _u32(), _u32()
+        self._L.vx_plot_launches(self._h, ctypes.byref(l1), ctypes.byref(l2))
+        self.launches_per_plot = l1.value + l2.value
         self.rec1_bytes = self.nonce_size + 8
         self.rec2_bytes = 2 * self.nonce_size
         need = int(self._L.vx_workspace_bytes_opts(K, bucket_bits, flags))

@@ -66,7 +66,24 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     }
     g->off_t1_off = o;    o = align256(o + (g->NB + 1) * 8);
     g->off_t2_off = o;    o = align256(o + (g->NB + 1) * 8);
-    g->off_t2_rec = o;    o = align256(o + g->t2_cap * (size_t)8);
+    size_t t2_bytes = g->t2_cap * (size_t)8;
+    if (g->wide) {
+        // stage 1 in rounds: 4 slices (K >= 2), scratch partitions one hash bit coarser than the
+        // final ones.  K = 33: slices of 2^31 nonces into 2^19 scratch partitions of ~4096 records,
+        // the geometry stage 1 runs ALU-bound in at K = 31.
+        g->round_log = K >= 2 ? K - 2 : K;
+        g->rounds = 1u << (K - g->round_log);
+        g->pb_tmp = g->pb ? g->pb - 1 : 0;
+        const uint64_t mean_tmp = (1ull << g->round_log) >> g->pb_tmp;
+        uint64_t cap_tmp = g->pb_tmp == 0 ? mean_tmp : mean_tmp + (uint64_t)ceil(8.0 * sqrt((double)mean_tmp));
+        cap_tmp = (cap_tmp + 31) & ~(uint64_t)31;
+        g->cap_tmp = (uint32_t)cap_tmp;
+        const size_t tmp_bytes = ((size_t)1 << g->pb_tmp) * cap_tmp * 16;
+        if (tmp_bytes > t2_bytes) t2_bytes = tmp_bytes;      // tiny K only
+        g->off_cursor_tmp = o; o = align256(o + ((size_t)4 << g->pb_tmp));
+    }
+    g->off_t2_rec = o;    o = align256(o + t2_bytes);
+    g->off_tmp = g->off_t2_rec;                              // scratch of stage 1, dead before stage 2
     if (g->wide) { g->off_t2_hi = o; o = align256(o + g->t2_cap); }
     g->stage_bytes = g->N * (size_t)g->rec1_bytes;
     if (g->stage_bytes > VX_STAGE_MAX_BYTES) g->stage_bytes = VX_STAGE_MAX_BYTES;
@@ -388,6 +405,14 @@ vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uin
     if (partition_bits) *partition_bits = p->g.pb;
     if (partition_capacity) *partition_capacity = p->g.cap;
     if (t2_capacity) *t2_capacity = p->g.t2_cap;
+    return VX_OK;
+}
+
+vx_status vx_plot_launches(const vx_plot *p, uint32_t *build_table1, uint32_t *sort_match_table2)
+{
+    if (!p) return VX_ERR_ARG;
+    if (build_table1) *build_table1 = vx_stage1_launches(p->g);
+    if (sort_match_table2) *sort_match_table2 = 1;
     return VX_OK;
 }
 

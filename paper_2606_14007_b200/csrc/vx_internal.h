@@ -47,6 +47,12 @@ struct VxGeom {
     size_t off_t1_off, off_t2_off, off_t2_rec;
     size_t off_t2_hi;  // wide only: uint8 per Table-2 record, (n1 >> 32) | (n2 >> 32) << 4
     size_t off_stage, stage_bytes;   // export staging for vx_read_tables(Table 1)
+    // wide only -- stage 1 in rounds: the nonce space is hashed in
+    // `rounds` slices of 2^round_log nonces; each slice is scattered as 16-byte records (one store
+    // request per record) into 2^pb_tmp coarse partitions of a scratch area that aliases the not yet
+    // used Table-2 region, then compacted into the 10-byte partition array with coalesced stores.
+    uint32_t rounds, round_log, pb_tmp, cap_tmp;
+    size_t off_cursor_tmp, off_tmp;
     size_t total;
 };
 
@@ -70,6 +76,7 @@ void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_s
 
 // ---------------------------------------------------------------------------------- launches
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st);
+uint32_t vx_stage1_launches(const VxGeom &g);   // kernels vx_launch_stage1 enqueues
 cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool force_exact, int num_sms,
                              cudaStream_t st);
 // external-format Table-1 records [first, first + count) of the CSR numbering -> ws + off_stage

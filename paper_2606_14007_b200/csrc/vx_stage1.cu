@@ -17,16 +17,15 @@
 #define VX_S1_THREADS 256
 #define VX_S1_NPT 4
 
-// WIDE (K >= 33, or forced by a test): the record is 10 bytes in two arrays with the same slot
-// numbering, a = (H << pb) | (n >> tile_log) (the partition prefix of H is implied by the partition, the
-// pb bits it frees hold the high nonce bits) and b = n & (2^tile_log - 1) -- DESIGN.md "wide layout".
-template <bool NONCE5, bool WIDE>
+// The record is one aligned 16-byte store {H lo, H hi, nonce lo, nonce hi}.  The wide layout
+// (K >= 33) runs this same kernel per round into its scratch partitions (vx_k_compact below).
+template <bool NONCE5>
 __global__ void __launch_bounds__(VX_S1_THREADS)
-vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t pb, uint32_t nlo_bits, uint32_t cap,
-                  uint4 *__restrict__ part, uint16_t *__restrict__ part_b,
-                  uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
+vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint64_t N, uint32_t pb, uint32_t cap,
+                  uint4 *__restrict__ part, uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
 {
-    const uint64_t base = (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
+    // nonces [n_begin, N): the whole plot, or one round of it (wide layout, vx_launch_stage1)
+    const uint64_t base = n_begin + (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
     uint64_t H[VX_S1_NPT];
 #pragma unroll
     for (int k = 0; k < VX_S1_NPT; k++) {
@@ -40,19 +39,72 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t N, uint32_t p
             const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
             const uint32_t slot = atomicAdd(&cursor[p], 1u);
             if (slot < cap) {
-                if constexpr (WIDE) {
-                    reinterpret_cast<uint64_t *>(part)[(uint64_t)p * cap + slot] = (H[k] << pb) | (n >> nlo_bits);
-                    part_b[(uint64_t)p * cap + slot] = (uint16_t)(n & ((1u << nlo_bits) - 1u));
-                } else {
-                    // one 16-byte store per record: scattered stores are bound by requests, not bytes
-                    part[(uint64_t)p * cap + slot] =
-                        make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)n, (uint32_t)(n >> 32));
-                }
+                // one 16-byte store per record: scattered stores are bound by requests, not bytes
+                part[(uint64_t)p * cap + slot] =
+                    make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)n, (uint32_t)(n >> 32));
             } else {
                 atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
             }
         }
     }
+}
+
+// ----------------------------------------------------------------------------- wide: compaction
+// Stage 1 in rounds (wide layout, K >= 33).  A 10-byte record written
+// straight from the hash kernel costs two scattered store requests plus the atomic, and scattered
+// stores are bound by requests: K=33 stage 1 ran 2.6x over its ALU bound that way.  Instead each
+// round scatters its slice as 16-byte records (ONE request each, the narrow kernel above) into
+// 2^pb_tmp scratch partitions, and this kernel moves every scratch partition into the 2^d final
+// partitions it covers (d = pb - pb_tmp) in the compact layout a = (H << pb) | (n >> nlo_bits),
+// b = n & (2^nlo_bits - 1): contiguous 16-byte loads, and stores that are contiguous per final
+// partition, so this pass runs at HBM speed (26 bytes per record).
+// One CTA per scratch partition; it is the only writer of its final partitions' cursors in this
+// round (rounds are serialised on the stream), so those are plain loads and stores.
+#define VX_CP_THREADS 256
+#define VX_CP_MAXSUB 4
+__global__ void __launch_bounds__(VX_CP_THREADS)
+vx_k_compact(const uint4 *__restrict__ tmp, const uint32_t *__restrict__ cursor_tmp, uint32_t cap_tmp,
+             uint32_t pb, uint32_t d, uint32_t nlo_bits, uint32_t cap,
+             unsigned long long *__restrict__ part_a, uint16_t *__restrict__ part_b,
+             uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
+{
+    __shared__ uint32_t s_base[VX_CP_MAXSUB], s_cnt[VX_CP_MAXSUB];
+    const uint32_t p = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const uint32_t nsub = 1u << d;
+    const uint32_t cnt_raw = cursor_tmp[p];
+    const uint32_t cnt = min(cnt_raw, cap_tmp);
+    if (tid < nsub) { s_base[tid] = cursor[(p << d) + tid]; s_cnt[tid] = 0u; }
+    if (tid == 0 && cnt_raw > cap_tmp) atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
+    __syncthreads();
+    const uint4 *src = tmp + (size_t)p * cap_tmp;
+    bool over = false;
+    for (uint32_t i0 = 0; i0 < cnt; i0 += VX_CP_THREADS) {
+        const uint32_t i = i0 + tid;
+        const bool valid = i < cnt;
+        const uint4 r = valid ? __ldcs(src + i) : make_uint4(0u, 0u, 0u, 0u);
+        const unsigned long long H = ((unsigned long long)r.y << 32) | r.x;
+        const unsigned long long n = ((unsigned long long)r.w << 32) | r.z;
+        const uint32_t s = d ? (uint32_t)(H >> (64 - pb)) & (nsub - 1u) : 0u;
+        // warp-aggregated slot claim, one shared atomic per (warp, final partition)
+        const unsigned peers = __match_any_sync(0xffffffffu, valid ? s : 0xffffffffu);
+        const int leader = __ffs(peers) - 1;
+        uint32_t off = 0;
+        if (valid && (int)lane == leader) off = atomicAdd(&s_cnt[s], (uint32_t)__popc(peers));
+        off = __shfl_sync(0xffffffffu, off, leader);
+        if (valid) {
+            const uint32_t slot = s_base[s] + off + __popc(peers & ((1u << lane) - 1u));
+            if (slot < cap) {
+                const size_t at = (size_t)((p << d) + s) * cap + slot;
+                part_a[at] = (H << pb) | (n >> nlo_bits);
+                part_b[at] = (uint16_t)(n & ((1u << nlo_bits) - 1u));
+            } else {
+                over = true;
+            }
+        }
+    }
+    if (over) atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
+    __syncthreads();
+    if (tid < nsub) cursor[(p << d) + tid] = s_base[tid] + s_cnt[tid];   // counts every claim, like stage 1's atomics
 }
 
 // Exclusive prefix sum of the clamped partition counts: part_base[p] = number of records in
@@ -149,6 +201,8 @@ vx_k_hash_sink(const __grid_constant__ VxHashConst hc, uint64_t count, uint64_t 
 }
 
 // ----------------------------------------------------------------------------- launches
+uint32_t vx_stage1_launches(const VxGeom &g) { return g.wide ? 2u * g.rounds + 1u : 2u; }
+
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st)
 {
     VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
@@ -158,17 +212,39 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
     e = cudaMemsetAsync(cursor, 0, g.P * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
-    const uint64_t grid = (g.N + per_cta - 1) / per_cta;
     uint4 *part = (uint4 *)(ws + g.off_part);
     uint16_t *part_b = (uint16_t *)(ws + g.off_part_b);
-    if (g.nonce_size == 5)
-        vx_k_hash_scatter<true, true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.tile_log, g.cap, part, part_b, cursor, ctrl);
-    else if (g.wide)
-        vx_k_hash_scatter<false, true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.tile_log, g.cap, part, part_b, cursor, ctrl);
-    else
-        vx_k_hash_scatter<false, false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, g.N, g.pb, g.tile_log, g.cap, part, part_b, cursor, ctrl);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    if (g.wide) {
+        // stage 1 in rounds: hash + one-request scatter of a slice into the scratch partitions
+        // (they alias the Table-2 region, unused until stage 2), then compaction into the 10-byte layout
+        if (g.pb - g.pb_tmp > 2 || (1u << (g.pb - g.pb_tmp)) > VX_CP_MAXSUB) return cudaErrorInvalidValue;
+        uint4 *tmp = (uint4 *)(ws + g.off_tmp);
+        uint32_t *cursor_tmp = (uint32_t *)(ws + g.off_cursor_tmp);
+        const uint64_t slice = 1ull << g.round_log;
+        const uint64_t grid = (slice + per_cta - 1) / per_cta;
+        for (uint32_t r = 0; r < g.rounds; r++) {
+            e = cudaMemsetAsync(cursor_tmp, 0, sizeof(uint32_t) << g.pb_tmp, st);
+            if (e != cudaSuccess) return e;
+            if (g.nonce_size == 5)
+                vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
+                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
+            else
+                vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
+                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            vx_k_compact<<<1u << g.pb_tmp, VX_CP_THREADS, 0, st>>>(
+                tmp, cursor_tmp, g.cap_tmp, g.pb, g.pb - g.pb_tmp, g.tile_log, g.cap,
+                (unsigned long long *)part, part_b, cursor, ctrl);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
+    } else {
+        const uint64_t grid = (g.N + per_cta - 1) / per_cta;
+        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, 0ull, g.N, g.pb, g.cap, part, cursor, ctrl);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap, g.P,
                                                        (unsigned long long *)(ws + g.off_part_base));
     return cudaGetLastError();
