@@ -252,25 +252,48 @@ def run_cuda(args):
     # ---- end to end through the C ABI with host buffers -----------------------------------
     # per step: key (32 B) in; Table 2 + its offsets out, streamed through a pinned staging buffer
     nb = 1 << BUCKET_BITS
-    chunks = args.e2e_chunks
-    per = nb // chunks
-    rec_cap = int(1.25 * plot.rec2_bytes * (N // chunks)) + (1 << 20)
-    pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
-    pinned_off = torch.empty(per + 1, dtype=torch.int64, pin_memory=True)
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     d2h = 0
+    streamed = plot.nonce_size == 4 and not args.e2e_serial
+    if streamed:
+        # vx_sort_match_table2_to_host: stage 2 in slices, each finished slice copied
+        # on a second stream straight into place in one pinned buffer while later slices are matched
+        copy_stream = torch.cuda.Stream()
+        rec_cap = plot.rec2_bytes * plot.t2_capacity
+        pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
+        pinned_off = torch.empty(nb + 1, dtype=torch.int64, pin_memory=True)
+        e2e_what = ("vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2_to_host(Table 2 + offsets into "
+                    f"pinned host memory on a second stream, {args.e2e_slices} slices overlapped with the matching)")
 
-    def e2e_step():
-        nonlocal d2h
-        p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace)  # key -> kernel params
-        p2.build_table1(stream)
-        p2.sort_match_table2(stream)
-        moved = 0
-        for c in range(chunks):
-            moved += p2.read_tables_into(2, c * per, (c + 1) * per, pinned_off.data_ptr(),
-                                         pinned_rec.data_ptr(), rec_cap) + (per + 1) * 8
-        d2h = moved
-        p2.free()
+        def e2e_step():
+            nonlocal d2h
+            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace)  # key -> kernel params
+            p2.build_table1(stream)
+            d2h = p2.sort_match_table2_to_host(copy_stream, pinned_rec.data_ptr(), rec_cap, pinned_off.data_ptr(),
+                                               slices=args.e2e_slices, stream=stream) + (nb + 1) * 8
+            p2.free()
+    else:
+        # 5-byte nonces (K = 33): Table 2 is resident in a packed form; vx_read_tables converts and
+        # copies it range by range after the plot
+        chunks = args.e2e_chunks
+        per = nb // chunks
+        rec_cap = int(1.25 * plot.rec2_bytes * (N // chunks)) + (1 << 20)
+        pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
+        pinned_off = torch.empty(per + 1, dtype=torch.int64, pin_memory=True)
+        e2e_what = ("vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2 + vx_read_tables(Table 2, "
+                    f"{chunks} bucket ranges) into pinned host memory")
+
+        def e2e_step():
+            nonlocal d2h
+            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace)  # key -> kernel params
+            p2.build_table1(stream)
+            p2.sort_match_table2(stream)
+            moved = 0
+            for c in range(chunks):
+                moved += p2.read_tables_into(2, c * per, (c + 1) * per, pinned_off.data_ptr(),
+                                             pinned_rec.data_ptr(), rec_cap) + (per + 1) * 8
+            d2h = moved
+            p2.free()
 
     e2e_step()                      # warm the pinned path
     barrier()
@@ -313,8 +336,7 @@ def run_cuda(args):
             "roofline": {k: dominant[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel", "peak_source", "traffic_source")},
             "e2e": {"value": world * N / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 32,
                     "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
-                    "what": "vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2 + vx_read_tables(Table 2, "
-                            f"{chunks} bucket ranges) into pinned host memory"},
+                    "what": e2e_what},
             "gpu_launches": plot.launches_per_plot * args.steps,
             "clocks": clocks,
         }
@@ -338,6 +360,9 @@ def main():
     ap.add_argument("--ref-K", dest="ref_K", type=int, default=22, help="oracle sample size per --impl reference step")
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=2)
     ap.add_argument("--e2e-chunks", dest="e2e_chunks", type=int, default=32)
+    ap.add_argument("--e2e-slices", dest="e2e_slices", type=int, default=16)
+    ap.add_argument("--e2e-serial", dest="e2e_serial", action="store_true",
+                    help="e2e with vx_read_tables after the plot instead of the streamed egress")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":

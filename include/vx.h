@@ -53,7 +53,8 @@ typedef enum {
     VX_ERR_CUDA = -4,      /* a CUDA runtime call failed; text in vx_last_error                    */
     VX_ERR_OVERFLOW = -5,  /* a partition's slack or the Table-2 capacity overflowed on the device */
     VX_ERR_RANGE = -6,     /* bucket range outside [0, 2^B] or records_capacity too small          */
-    VX_ERR_UNSUPPORTED = -7 /* reserved: a valid configuration this build does not implement        */
+    VX_ERR_UNSUPPORTED = -7, /* a valid configuration this call does not implement                    */
+    VX_ERR_IO = -8          /* write() to the egress file descriptor failed; text in vx_last_error    */
 } vx_status;
 
 /* Device bytes the caller must provide for a plot of this K (B = 24 buckets bits, the paper's
@@ -99,6 +100,30 @@ vx_status vx_build_table1(vx_plot *p, void *cuda_stream);
  * Table 1 in place (reading A14) and the matches to Table 2, with exact CSR offsets for both.
  * Enqueues only. */
 vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream);
+
+/* Table-2 egress pipeline ("transferred from VRAM to host over PCIe and
+ * written to disk in 4 MB sequential chunks", L91 pinned staging buffer, L165/L169 "overlap the PCIe
+ * transfer with GPU computation using async streams").  Both calls replace vx_sort_match_table2: the
+ * fused sort + match stage runs as `slices` launches over consecutive partition ranges on
+ * compute_stream (1..256; clamped), and the Table-2 records and CSR offsets of each finished slice
+ * are copied on copy_stream (a different stream) while the later slices are still being matched.
+ * Both BLOCK until everything has arrived and report device-raised errors like vx_synchronize.
+ * K <= 32 only (VX_ERR_UNSUPPORTED for 5-byte nonces, whose Table 2 is resident in a packed form).
+ *
+ * _to_host: host_records (HOST, caller-owned, pinned for the copies to overlap; records_capacity
+ *   bytes, VX_ERR_RANGE if too small) receives all of Table 2 in the external format, bucket-major;
+ *   host_offsets (HOST, 2^B + 1 entries, may be NULL) the CSR offsets; *records_bytes the size.
+ * _to_file: the same stream of bytes goes to file descriptor fd with sequential write()s of 4 MB
+ *   through pinned_staging (HOST, pinned, caller-owned, >= 8 MB; used as a ring of 4 MB chunks, up
+ *   to 1024 of them): records, then the (2^B + 1) uint64 offsets, then a 32-byte trailer
+ *   {"VXT2\0\0\0\1", u32 K, u32 B, u32 NONCE_SIZE, u32 0, u64 |Table 2|}.  The paper's plot-file
+ *   format is unpublished; this layout is this library's own.  *file_bytes = bytes
+ *   written.  VX_ERR_IO if a write fails. */
+vx_status vx_sort_match_table2_to_host(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                                       void *host_records, size_t records_capacity, uint64_t *host_offsets,
+                                       size_t *records_bytes);
+vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                                       int fd, void *pinned_staging, size_t staging_bytes, uint64_t *file_bytes);
 
 /* Copy the buckets [bucket_begin, bucket_end) of table 1 or 2 to HOST memory in the external
  * format.  Synchronises the plot's stream.  offsets_out (may be NULL) receives

@@ -18,12 +18,13 @@ VX_OPT_FORCE_EXACT_RANK = 1
 VX_CREATE_WIDE_LAYOUT = 1
 VX_CREATE_BIG_TILES = 2
 STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",
-          -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED"}
+          -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED", -8: "VX_ERR_IO"}
 
 #: every symbol include/vx.h declares
 EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_opts", "vx_plot_create",
            "vx_plot_create_ex", "vx_plot_create_opts",
-           "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_read_tables",
+           "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
+           "vx_sort_match_table2_to_file", "vx_read_tables",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
@@ -78,6 +79,10 @@ def load_library() -> ctypes.CDLL:
     L.vx_build_table1.argtypes = [_vp, _vp]
     L.vx_sort_match_table2.restype = ctypes.c_int
     L.vx_sort_match_table2.argtypes = [_vp, _vp]
+    L.vx_sort_match_table2_to_host.restype = ctypes.c_int
+    L.vx_sort_match_table2_to_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _sz, _vp, ctypes.POINTER(_sz)]
+    L.vx_sort_match_table2_to_file.restype = ctypes.c_int
+    L.vx_sort_match_table2_to_file.argtypes = [_vp, _vp, _vp, _u32, ctypes.c_int, _vp, _sz, ctypes.POINTER(_u64)]
     L.vx_read_tables.restype = ctypes.c_int
     L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
     L.vx_device_tables.restype = ctypes.c_int
@@ -189,6 +194,25 @@ class Plot:
 
     def sort_match_table2(self, stream=None):
         self._check(self._L.vx_sort_match_table2(self._h, _stream_ptr(stream)))
+
+    def sort_match_table2_to_host(self, copy_stream, records_ptr: int, records_capacity: int,
+                                  offsets_ptr: int = 0, slices: int = 16, stream=None) -> int:
+        """Stage 2 in `slices` launches with Table 2 streamed to host memory on copy_stream
+        (vx_sort_match_table2_to_host); raw host pointers (pinned torch tensors); returns record bytes."""
+        need = _sz()
+        self._check(self._L.vx_sort_match_table2_to_host(
+            self._h, _stream_ptr(stream), _stream_ptr(copy_stream), slices, records_ptr, records_capacity,
+            offsets_ptr or None, ctypes.byref(need)))
+        return need.value
+
+    def sort_match_table2_to_file(self, copy_stream, fd: int, staging_ptr: int, staging_bytes: int,
+                                  slices: int = 16, stream=None) -> int:
+        """Same, to a file descriptor through a pinned ring of 4 MB chunks; returns the bytes written."""
+        n = _u64()
+        self._check(self._L.vx_sort_match_table2_to_file(
+            self._h, _stream_ptr(stream), _stream_ptr(copy_stream), slices, fd, staging_ptr, staging_bytes,
+            ctypes.byref(n)))
+        return n.value
 
     def synchronize(self):
         self._check(self._L.vx_synchronize(self._h))

@@ -4,6 +4,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <unistd.h>
 
 #include <new>
 
@@ -165,6 +166,7 @@ const char *vx_status_string(vx_status s)
     case VX_ERR_OVERFLOW: return "VX_ERR_OVERFLOW";
     case VX_ERR_RANGE: return "VX_ERR_RANGE";
     case VX_ERR_UNSUPPORTED: return "VX_ERR_UNSUPPORTED";
+    case VX_ERR_IO: return "VX_ERR_IO";
     }
     return "VX_ERR_?";
 }
@@ -335,6 +337,72 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
         if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(exported records)");
     }
     return VX_OK;
+}
+
+// ------------------------------------------------------------------------------ egress (8(f1))
+static vx_status egress_common(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                               uint8_t *host_records, size_t records_capacity, uint64_t *host_offsets,
+                               VxRing *ring, uint64_t *t2_records)
+{
+    if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "Table-2 egress before vx_build_table1");
+    if (p->g.nonce_size > 4)
+        return fail(p, VX_ERR_UNSUPPORTED, "streamed egress needs Table 2 resident in the external format (K <= 32)");
+    if (compute_stream == copy_stream) return fail(p, VX_ERR_ARG, "compute and copy streams must differ");
+    p->stream = (cudaStream_t)compute_stream;
+    int soft = 0;
+    char msg[256] = "";
+    cudaError_t e = vx_egress_run(p->g, p->ws, p->force_exact, p->num_sms, p->stream, (cudaStream_t)copy_stream,
+                                  slices, host_records, records_capacity, host_offsets, ring, t2_records, &soft,
+                                  msg, sizeof msg);
+    if (e != cudaSuccess) return fail_cuda(p, e, "Table-2 egress");
+    p->state = VX_MATCHED;
+    p->t1_materialised = true;
+    if (soft == 1) return fail(p, VX_ERR_RANGE, msg);
+    if (soft == 2) return fail(p, VX_ERR_OVERFLOW, msg);
+    if (soft == 3) return fail(p, VX_ERR_IO, msg);
+    return sync_and_check(p);
+}
+
+vx_status vx_sort_match_table2_to_host(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                                       void *host_records, size_t records_capacity, uint64_t *host_offsets,
+                                       size_t *records_bytes)
+{
+    if (!p) return VX_ERR_ARG;
+    if (!host_records) return fail(p, VX_ERR_ARG, "NULL host_records");
+    uint64_t n = 0;
+    vx_status s = egress_common(p, compute_stream, copy_stream, slices, (uint8_t *)host_records, records_capacity,
+                                host_offsets, NULL, &n);
+    if (records_bytes) *records_bytes = (size_t)n * p->g.rec2_bytes;
+    return s;
+}
+
+vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                                       int fd, void *pinned_staging, size_t staging_bytes, uint64_t *file_bytes)
+{
+    if (!p) return VX_ERR_ARG;
+    if (fd < 0 || !pinned_staging) return fail(p, VX_ERR_ARG, "bad file descriptor or NULL staging buffer");
+    VxRing *ring = vx_ring_create(pinned_staging, staging_bytes, fd);
+    if (!ring) return fail(p, VX_ERR_ARG, "staging buffer smaller than two 4 MB chunks");
+    uint64_t n = 0;
+    vx_status s = egress_common(p, compute_stream, copy_stream, slices, NULL, 0, NULL, ring, &n);
+    uint64_t written = vx_ring_written(ring);
+    vx_ring_destroy(ring);
+    if (s == VX_OK) {
+        // trailer: magic, K, B, NONCE_SIZE, reserved, |Table 2|  (all little-endian)
+        uint8_t tr[32] = {'V', 'X', 'T', '2', 0, 0, 0, 1};
+        const uint32_t w[4] = {p->g.K, p->g.B, p->g.nonce_size, 0u};
+        memcpy(tr + 8, w, 16);
+        memcpy(tr + 24, &n, 8);
+        size_t left = sizeof tr;
+        const uint8_t *src = tr;
+        while (left) {
+            const ssize_t k = write(fd, src, left);
+            if (k < 0) return fail(p, VX_ERR_IO, "write(trailer) failed");
+            src += k; left -= (size_t)k; written += (uint64_t)k;
+        }
+    }
+    if (file_bytes) *file_bytes = written;
+    return s;
 }
 
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,

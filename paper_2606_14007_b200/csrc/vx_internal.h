@@ -77,8 +77,12 @@ void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_s
 // ---------------------------------------------------------------------------------- launches
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st);
 uint32_t vx_stage1_launches(const VxGeom &g);   // kernels vx_launch_stage1 enqueues
+// sorts (and matches) the partitions [tile_begin, tile_end) -- (0, P) for the whole plot; slices must
+// be launched in ascending order on one stream.  slice_end_out (host-mapped, may be NULL) receives
+// the number of Table-2 records of the partitions < tile_end.
 cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool force_exact, int num_sms,
-                             cudaStream_t st);
+                             cudaStream_t st, uint32_t tile_begin = 0, uint32_t tile_end = 0xffffffffu,
+                             unsigned long long *slice_end_out = nullptr);
 // external-format Table-1 records [first, first + count) of the CSR numbering -> ws + off_stage
 cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
 // wide, NONCE_SIZE = 5: external 10-byte Table-2 records [first, first + count) -> ws + off_stage
@@ -87,5 +91,16 @@ cudaError_t vx_launch_hash_range(const VxGeom &g, const VxHashConst &hc, uint64_
                                  uint64_t count, uint64_t *dev_hashes, cudaStream_t st);
 cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t count,
                                 uint64_t *dev_sink, size_t sink_words, cudaStream_t st);
+// Table-2 egress (vx_egress.cu): stage 2 in `slices` partition-range launches on `compute`, each
+// finished slice copied on `copy` to host memory (host_records / host_offsets) or, through a pinned
+// ring of 4 MB chunks, to a file.  *soft_error: 0 ok, 1 capacity too small, 2 Table-2 overflow, 3 I/O.
+struct VxRing;
+VxRing *vx_ring_create(void *pinned, size_t bytes, int fd);   // NULL: fewer than two 4 MB chunks, or no memory
+uint64_t vx_ring_written(const VxRing *r);
+void vx_ring_destroy(VxRing *r);
+cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int num_sms, cudaStream_t compute,
+                          cudaStream_t copy, uint32_t slices, uint8_t *host_records, size_t records_capacity,
+                          uint64_t *host_offsets, VxRing *ring, uint64_t *t2_records, int *soft_error,
+                          char *err, size_t errlen);
 cudaError_t vx_stage2_configure(void); // opt in to the large dynamic shared memory once
 size_t vx_stage2_smem_bytes(const VxGeom &g);

@@ -46,6 +46,10 @@ struct VxS2Params {
     unsigned long long *t2_off;
     unsigned long long N, NB, t2_cap;
     uint32_t P, cap, pb, fb, K, B, do_match, force_exact;
+    // this launch sorts the partitions [tile_begin, tile_end): the whole plot, or one slice of it
+    // when Table 2 is streamed to the host while later slices are still being matched (vx_egress.cu)
+    uint32_t tile_begin, tile_end;
+    unsigned long long *slice_end_out;   // host-mapped: |Table 2| after partition tile_end - 1, or NULL
 };
 
 #define VX_ST_AGG (1ull << 62)
@@ -182,7 +186,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
     for (;;) {
         __syncthreads();                                // previous tile fully drained
-        if (tid == 0) s_tile = atomicAdd(&q.ctrl->ticket, 1u);
+        if (tid == 0) s_tile = q.tile_begin + atomicAdd(&q.ctrl->ticket, 1u);
         // exact = rank by (H, n) with full compares; the fast pass ranks by H alone and is
         // validated in phase E (a tile holding two equal hashes comes back for an exact pass)
         uint32_t exact = q.force_exact | (q.do_match ^ 1u);
@@ -201,7 +205,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             __syncthreads();
             if (tid == 0) s_tie = 0u;                   // set in phase E, read after the sync behind it
             tile = s_tile;
-            if (tile >= q.P) { finished = true; break; }
+            if (tile >= q.tile_end) { finished = true; break; }
             cnt = min(q.cursor[tile], q.cap);
             base1 = q.part_base[tile];
             if constexpr (WIDE) {
@@ -410,7 +414,10 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             // ---- look-back for the Table-2 base ----------------------------------------------------
             if (tid < 32) {
                 const unsigned long long b2 = vx_lookback(q.status, tile, M, lane);
-                if (tid == 0) s_base2 = b2;
+                if (tid == 0) {
+                    s_base2 = b2;
+                    if (tile == q.tile_end - 1 && q.slice_end_out) *q.slice_end_out = b2 + M;
+                }
             }
             __syncthreads();
             base2 = s_base2;
@@ -581,15 +588,20 @@ cudaError_t vx_stage2_configure(void)
 }
 
 cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool force_exact, int num_sms,
-                             cudaStream_t st)
+                             cudaStream_t st, uint32_t tile_begin, uint32_t tile_end,
+                             unsigned long long *slice_end_out)
 {
     VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
+    if (tile_end > g.P) tile_end = (uint32_t)g.P;
+    if (tile_begin >= tile_end) return cudaErrorInvalidValue;
     cudaError_t e = cudaMemsetAsync(&ctrl->ticket, 0, sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(&ctrl->max_bucket, 0, sizeof(uint32_t), st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(ws + g.off_status, 0, g.P * sizeof(unsigned long long), st);
-    if (e != cudaSuccess) return e;
+    if (tile_begin == 0) {                              // first (or only) slice of the plot
+        e = cudaMemsetAsync(&ctrl->max_bucket, 0, sizeof(uint32_t), st);
+        if (e != cudaSuccess) return e;
+        e = cudaMemsetAsync(ws + g.off_status, 0, g.P * sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return e;
+    }
     VxS2Params q;
     q.part = (uint4 *)(ws + g.off_part);
     q.cursor = (const uint32_t *)(ws + g.off_cursor);
@@ -603,6 +615,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
+    q.tile_begin = tile_begin; q.tile_end = tile_end; q.slice_end_out = slice_end_out;
     if (g.pb + g.tile_log > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
     q.part_b = (uint16_t *)(ws + g.off_part_b);
     q.t2_hi = ws + g.off_t2_hi;
@@ -625,7 +638,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.nlo_bits = g.tile_log;
     const bool big = g.tile_log == VX_TILE_LOG_BIG;
     uint64_t grid = (uint64_t)num_sms * (big ? 1 : VX_S2_MINB);
-    if (grid > g.P) grid = g.P;
+    if (grid > tile_end - tile_begin) grid = tile_end - tile_begin;
     if (big && g.wide) VX_S2B_KERNEL(true)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
     else if (big) VX_S2B_KERNEL(false)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
     else if (g.wide) VX_S2_KERNEL(true)<<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
