@@ -32,7 +32,8 @@ def is_stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/*.cu into paper_2606_14007_b200/libvx.so; returns its path."""
     if force or is_stale():
-        cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
+        extra = os.environ.get("VX_NVCC_EXTRA", "").split()      # e.g. -DVX_S1_ITERS=4 (experiments)
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
                *[os.path.join(CSRC, s) for s in SOURCES]]
         subprocess.check_call(cmd, cwd=CSRC)
     return LIB

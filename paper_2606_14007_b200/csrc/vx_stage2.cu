@@ -175,6 +175,10 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_tile, s_tie;
     __shared__ unsigned long long s_base2;
+    // deferred emit (phase H of tile t runs after phase A of the CTA's next tile): Table-2 prefix at
+    // the first record of every bucket of tile t, saved before the bins are recycled
+    constexpr uint32_t VX_DEFER_MAXB = 512;
+    __shared__ uint32_t s_e2[VX_DEFER_MAXB];
 
     const int tid = threadIdx.x, lane = tid & 31, wbase = tid & ~31;
     const int sh = q.binshift - 32;                     // bin / sub-key shifts act on the high key word
@@ -183,6 +187,64 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     const uint64_t Tm1 = q.Tm1;                         // T - 1 in key units
     const uint64_t bmask = q.bmask;                     // key | bmask = last key of the key's bucket
     uint32_t cta_max_bucket = 0;
+    const uint32_t nb_local = 1u << q.fb;
+    // The Table-2 base of a tile comes from the decoupled look-back over all earlier tiles, and the
+    // ~300 tiles in flight run a few microseconds apart: emitting right after the write-back left
+    // the CTA waiting 13 % of its time.  So a tile's look-back + emit (phase H) are deferred until
+    // the CTA has loaded and binned its NEXT tile (phase A touches only registers and the bins):
+    // the predecessors get that much longer to publish their totals.
+    const bool defer = q.do_match && nb_local <= VX_DEFER_MAXB;
+    bool pending = false;                               // CTA-uniform
+    uint32_t p_tile = 0, p_cnt = 0, p_M = 0;
+
+    // ---- look-back for the Table-2 base, then H: the matches of i are i+1 .. i+c_i, c_i = E[i+1] - E[i]
+    auto lookback_emit = [&](uint32_t tile, uint32_t cnt, uint32_t M) {
+        if (tid < 32) {
+            const unsigned long long b2 = vx_lookback(q.status, tile, M, lane);
+            if (tid == 0) {
+                s_base2 = b2;
+                if (tile == q.tile_end - 1 && q.slice_end_out) *q.slice_end_out = b2 + M;
+            }
+        }
+        __syncthreads();
+        const unsigned long long base2 = s_base2;
+        if (base2 + M > q.t2_cap) {
+            if (tid == 0) atomicOr(&q.ctrl->flags, VX_FLAG_T2_OVERFLOW);
+        } else {
+#pragma unroll
+            for (int it = 0; it < ITEMS; it++) {
+                if (it * THREADS + wbase < cnt) {
+                    const uint32_t i = it * THREADS + tid;
+                    const uint32_t e0 = E[i];
+                    const uint32_t c = E[i + 1] - e0;
+                    const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
+                    if (cmax) {
+                        if constexpr (WIDE) {
+                            // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key
+                            const uint64_t ni = ((keyS[i] & q.lowmask) << q.nlo_bits) | nonS[i];
+                            const unsigned long long at = base2 + e0;
+                            for (uint32_t t = 0; t < cmax; t++)
+                                if (t < c) {
+                                    const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << q.nlo_bits) | nonS[i + 1 + t];
+                                    q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
+                                    q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
+                                }
+                        } else {
+                            const uint32_t ni = nonS[i];
+                            const uint32_t *np = nonS + i + 1;
+                            uint2 *dst = q.t2_rec + (base2 + e0);
+#pragma unroll
+                            for (uint32_t t = 0; t < 4; t++)
+                                if (t < c) dst[t] = make_uint2(ni, np[t]);
+                            for (uint32_t t = 4; t < cmax; t++)
+                                if (t < c) dst[t] = make_uint2(ni, np[t]);
+                        }
+                    }
+                }
+            }
+        }
+        return base2;
+    };
 
     for (;;) {
         __syncthreads();                                // previous tile fully drained
@@ -196,7 +258,6 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         unsigned short *src_b = nullptr;
         uint64_t key[ITEMS];
         uint32_t non[ITEMS], sn[ITEMS];                 // sn: slot, later position | bin size << 16
-        uint32_t cc[ITEMS];
         uint32_t M = 0;
         bool finished = false;
         for (;;) {
@@ -205,9 +266,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             __syncthreads();
             if (tid == 0) s_tie = 0u;                   // set in phase E, read after the sync behind it
             tile = s_tile;
-            if (tile >= q.tile_end) { finished = true; break; }
-            cnt = min(q.cursor[tile], q.cap);
-            base1 = q.part_base[tile];
+            const bool valid = tile < q.tile_end;
+            cnt = valid ? min(q.cursor[tile], q.cap) : 0u;
+            base1 = valid ? q.part_base[tile] : 0ull;
             if constexpr (WIDE) {
                 src = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned long long *>(q.part) + (size_t)tile * q.cap);
                 src_b = q.part_b + (size_t)tile * q.cap;
@@ -233,6 +294,17 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 const uint32_t idx = it * THREADS + tid;
                 if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin<VX_NBINS>(key[it], sh)], 1u);
             }
+            if (pending) {                              // the previous tile of this CTA: look-back + H
+                const unsigned long long base2 = lookback_emit(p_tile, p_cnt, p_M);
+                const unsigned long long pg0 = (unsigned long long)p_tile << q.fb;
+                for (uint32_t bl = tid; bl < nb_local; bl += THREADS) q.t2_off[pg0 + bl] = base2 + s_e2[bl];
+                if (p_tile == q.P - 1 && tid == 0) {
+                    q.t2_off[q.NB] = base2 + p_M;
+                    q.ctrl->t2_total = base2 + p_M;
+                }
+                pending = false;
+            }
+            if (!valid) { finished = true; break; }
             __syncthreads();
             // ---- B. scan -------------------------------------------------------------------------
             {
@@ -354,7 +426,6 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             }
                         }
                     }
-                    cc[it] = c;
                     E[i] = c;
                 }
             }
@@ -375,7 +446,6 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             return s;
         };
 
-        unsigned long long base2 = 0;
         if (q.do_match) {
             // ---- F. scan, publish the aggregate ---------------------------------------------------
             M = vx_block_exscan<THREADS, ITEMS>(E, s_warp);
@@ -401,66 +471,26 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 }
             }
         }
-        const uint32_t nb_local = 1u << q.fb;
         const unsigned long long gb0 = (unsigned long long)tile << q.fb;
         for (uint32_t bl = tid; bl < nb_local; bl += THREADS) {
             const uint32_t s = bucket_start(bl), e = bucket_start(bl + 1);
             cta_max_bucket = max(cta_max_bucket, e - s);
             q.t1_off[gb0 + bl] = base1 + s;
+            if (defer) s_e2[bl] = E[s];
         }
         if (tile == q.P - 1 && tid == 0) q.t1_off[q.NB] = base1 + cnt;
 
         if (q.do_match) {
-            // ---- look-back for the Table-2 base ----------------------------------------------------
-            if (tid < 32) {
-                const unsigned long long b2 = vx_lookback(q.status, tile, M, lane);
-                if (tid == 0) {
-                    s_base2 = b2;
-                    if (tile == q.tile_end - 1 && q.slice_end_out) *q.slice_end_out = b2 + M;
-                }
-            }
-            __syncthreads();
-            base2 = s_base2;
-            // ---- H. emit: the matches of i are i+1 .. i+c_i ------------------------------------------
-            if (base2 + M > q.t2_cap) {
-                if (tid == 0) atomicOr(&q.ctrl->flags, VX_FLAG_T2_OVERFLOW);
+            if (defer) {
+                pending = true; p_tile = tile; p_cnt = cnt; p_M = M;
             } else {
-#pragma unroll
-                for (int it = 0; it < ITEMS; it++) {
-                    if (it * THREADS + wbase < cnt) {
-                        const uint32_t i = it * THREADS + tid;
-                        const uint32_t c = cc[it];
-                        const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
-                        if (cmax) {
-                            if constexpr (WIDE) {
-                                // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key
-                                const uint64_t ni = ((keyS[i] & q.lowmask) << q.nlo_bits) | nonS[i];
-                                const unsigned long long at = base2 + E[i];
-                                for (uint32_t t = 0; t < cmax; t++)
-                                    if (t < c) {
-                                        const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << q.nlo_bits) | nonS[i + 1 + t];
-                                        q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
-                                        q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
-                                    }
-                            } else {
-                                const uint32_t ni = nonS[i];
-                                const uint32_t *np = nonS + i + 1;
-                                uint2 *dst = q.t2_rec + (base2 + E[i]);
-#pragma unroll
-                                for (uint32_t t = 0; t < 4; t++)
-                                    if (t < c) dst[t] = make_uint2(ni, np[t]);
-                                for (uint32_t t = 4; t < cmax; t++)
-                                    if (t < c) dst[t] = make_uint2(ni, np[t]);
-                            }
-                        }
-                    }
+                const unsigned long long base2 = lookback_emit(tile, cnt, M);
+                for (uint32_t bl = tid; bl < nb_local; bl += THREADS)
+                    q.t2_off[gb0 + bl] = base2 + E[bucket_start(bl)];
+                if (tile == q.P - 1 && tid == 0) {
+                    q.t2_off[q.NB] = base2 + M;
+                    q.ctrl->t2_total = base2 + M;
                 }
-            }
-            for (uint32_t bl = tid; bl < nb_local; bl += THREADS)
-                q.t2_off[gb0 + bl] = base2 + E[bucket_start(bl)];
-            if (tile == q.P - 1 && tid == 0) {
-                q.t2_off[q.NB] = base2 + M;
-                q.ctrl->t2_total = base2 + M;
             }
         }
     }
