@@ -162,6 +162,12 @@ vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64
  * (H, n) re-ranking path it otherwise takes only for a tile holding two equal 64-bit hashes
  * (reading A10) -- results are identical by construction; tests use it to cover that path. */
 #define VX_OPT_FORCE_EXACT_RANK 1
+/* VX_OPT_PARTITION_CAPACITY_LIMIT (1 .. partition_capacity) / VX_OPT_TABLE2_CAPACITY_LIMIT
+ * (0 .. t2_capacity): lower the capacity the kernels CHECK against, without changing the layout,
+ * so that the overflow path can be exercised: the run then ends in VX_ERR_OVERFLOW at the next
+ * synchronising call instead of dropping records silently (reading A8). */
+#define VX_OPT_PARTITION_CAPACITY_LIMIT 2
+#define VX_OPT_TABLE2_CAPACITY_LIMIT 3
 vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value);
 
 /* Synchronises; any output pointer may be NULL.  max_bucket = largest Table-1 bucket. */

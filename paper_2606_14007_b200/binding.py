@@ -15,6 +15,8 @@ from . import build as _build
 
 VX_OK = 0
 VX_OPT_FORCE_EXACT_RANK = 1
+VX_OPT_PARTITION_CAPACITY_LIMIT = 2
+VX_OPT_TABLE2_CAPACITY_LIMIT = 3
 VX_CREATE_WIDE_LAYOUT = 1
 VX_CREATE_BIG_TILES = 2
 STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",

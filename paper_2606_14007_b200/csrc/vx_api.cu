@@ -50,8 +50,10 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     cap = (cap + 31) & ~(uint64_t)31;
     if (cap > (g->tile_log == VX_TILE_LOG_BIG ? VX_S2B_THREADS * VX_S2B_ITEMS : VX_S2_THREADS * VX_S2_ITEMS)) return false;
     g->cap = (uint32_t)cap;
+    g->cap_check = g->cap;
     // |T2| ~ 2^K (1 - 2^(B-K-1)) for K >= B, 2^(2K-1-B) below; sd ~ sqrt: 2^K + slack is ample
     g->t2_cap = g->N + (1u << 16);
+    g->t2_check = g->t2_cap;
     g->rec1_bytes = g->nonce_size + 8;
     g->rec2_bytes = 2 * g->nonce_size;
     size_t o = 0;
@@ -424,6 +426,14 @@ vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value)
     if (!p) return VX_ERR_ARG;
     switch (option) {
     case VX_OPT_FORCE_EXACT_RANK: p->force_exact = value != 0; return VX_OK;
+    case VX_OPT_PARTITION_CAPACITY_LIMIT:
+        if (value < 1 || value > p->g.cap) return fail(p, VX_ERR_ARG, "limit outside [1, partition capacity]");
+        p->g.cap_check = (uint32_t)value;
+        return VX_OK;
+    case VX_OPT_TABLE2_CAPACITY_LIMIT:
+        if (value > p->g.t2_cap) return fail(p, VX_ERR_ARG, "limit above the Table-2 capacity");
+        p->g.t2_check = value;
+        return VX_OK;
     }
     return fail(p, VX_ERR_ARG, "unknown option");
 }

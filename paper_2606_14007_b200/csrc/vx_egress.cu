@@ -103,7 +103,7 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
         const uint64_t cur = ends[s];
         const uint32_t t0 = (uint32_t)(P * s / slices), t1 = (uint32_t)(P * (s + 1) / slices);
         const uint64_t b0 = (uint64_t)t0 << g.fb, b1 = (uint64_t)t1 << g.fb;
-        if (cur < prev || cur > g.t2_cap) { snprintf(err, errlen, "Table 2 exceeded its capacity"); *soft_error = 2; break; }
+        if (cur < prev || cur > g.t2_check) { snprintf(err, errlen, "Table 2 exceeded its capacity"); *soft_error = 2; break; }
         if (host_records) {
             if (cur * rb > records_capacity) { snprintf(err, errlen, "records_capacity too small"); *soft_error = 1; break; }
             if (cur > prev)

@@ -32,6 +32,8 @@ struct VxGeom {
     uint32_t pb;   // partition bits: partition = H >> (64 - pb)
     uint32_t fb;   // bucket bits inside a partition, B - pb
     uint32_t cap;  // partition capacity in records (mean + slack, multiple of 32)
+    uint32_t cap_check;   // = cap; a test hook lowers it (the slot stride stays cap) to raise the overflow error
+    uint64_t t2_check;    // = t2_cap; likewise for Table 2
     uint64_t N;    // 2^K
     uint64_t P;    // 2^pb
     uint64_t NB;   // 2^B

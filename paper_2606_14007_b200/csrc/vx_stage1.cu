@@ -22,7 +22,8 @@
 template <bool NONCE5>
 __global__ void __launch_bounds__(VX_S1_THREADS)
 vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint64_t N, uint32_t pb, uint32_t cap,
-                  uint4 *__restrict__ part, uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
+                  uint32_t cap_check, uint4 *__restrict__ part, uint32_t *__restrict__ cursor,
+                  VxCtrl *__restrict__ ctrl)
 {
     // nonces [n_begin, N): the whole plot, or one round of it (wide layout, vx_launch_stage1)
     const uint64_t base = n_begin + (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
@@ -38,7 +39,7 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint
         if (n < N) {
             const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
             const uint32_t slot = atomicAdd(&cursor[p], 1u);
-            if (slot < cap) {
+            if (slot < cap_check) {                     // = cap, unless a test lowered it
                 // one 16-byte store per record: scattered stores are bound by requests, not bytes
                 part[(uint64_t)p * cap + slot] =
                     make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)n, (uint32_t)(n >> 32));
@@ -64,7 +65,7 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint
 #define VX_CP_MAXSUB 4
 __global__ void __launch_bounds__(VX_CP_THREADS)
 vx_k_compact(const uint4 *__restrict__ tmp, const uint32_t *__restrict__ cursor_tmp, uint32_t cap_tmp,
-             uint32_t pb, uint32_t d, uint32_t nlo_bits, uint32_t cap,
+             uint32_t pb, uint32_t d, uint32_t nlo_bits, uint32_t cap, uint32_t cap_check,
              unsigned long long *__restrict__ part_a, uint16_t *__restrict__ part_b,
              uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
 {
@@ -93,7 +94,7 @@ vx_k_compact(const uint4 *__restrict__ tmp, const uint32_t *__restrict__ cursor_
         off = __shfl_sync(0xffffffffu, off, leader);
         if (valid) {
             const uint32_t slot = s_base[s] + off + __popc(peers & ((1u << lane) - 1u));
-            if (slot < cap) {
+            if (slot < cap_check) {
                 const size_t at = (size_t)((p << d) + s) * cap + slot;
                 part_a[at] = (H << pb) | (n >> nlo_bits);
                 part_b[at] = (uint16_t)(n & ((1u << nlo_bits) - 1u));
@@ -227,25 +228,25 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
             if (e != cudaSuccess) return e;
             if (g.nonce_size == 5)
                 vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
-                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
+                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
             else
                 vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
-                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
+                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;
             vx_k_compact<<<1u << g.pb_tmp, VX_CP_THREADS, 0, st>>>(
-                tmp, cursor_tmp, g.cap_tmp, g.pb, g.pb - g.pb_tmp, g.tile_log, g.cap,
+                tmp, cursor_tmp, g.cap_tmp, g.pb, g.pb - g.pb_tmp, g.tile_log, g.cap, g.cap_check,
                 (unsigned long long *)part, part_b, cursor, ctrl);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;
         }
     } else {
         const uint64_t grid = (g.N + per_cta - 1) / per_cta;
-        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, 0ull, g.N, g.pb, g.cap, part, cursor, ctrl);
+        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, 0ull, g.N, g.pb, g.cap, g.cap_check, part, cursor, ctrl);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap, g.P,
+    vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap_check, g.P,
                                                        (unsigned long long *)(ws + g.off_part_base));
     return cudaGetLastError();
 }

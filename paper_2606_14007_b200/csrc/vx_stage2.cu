@@ -49,6 +49,7 @@ struct VxS2Params {
     // this launch sorts the partitions [tile_begin, tile_end): the whole plot, or one slice of it
     // when Table 2 is streamed to the host while later slices are still being matched (vx_egress.cu)
     uint32_t tile_begin, tile_end;
+    uint32_t cap_check;          // records a partition may hold (= cap unless a test lowered it)
     unsigned long long *slice_end_out;   // host-mapped: |Table 2| after partition tile_end - 1, or NULL
 };
 
@@ -267,7 +268,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             if (tid == 0) s_tie = 0u;                   // set in phase E, read after the sync behind it
             tile = s_tile;
             const bool valid = tile < q.tile_end;
-            cnt = valid ? min(q.cursor[tile], q.cap) : 0u;
+            cnt = valid ? min(q.cursor[tile], q.cap_check) : 0u;
             base1 = valid ? q.part_base[tile] : 0ull;
             if constexpr (WIDE) {
                 src = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned long long *>(q.part) + (size_t)tile * q.cap);
@@ -641,8 +642,8 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.t1_off = (unsigned long long *)(ws + g.off_t1_off);
     q.t2_rec = (uint2 *)(ws + g.off_t2_rec);
     q.t2_off = (unsigned long long *)(ws + g.off_t2_off);
-    q.N = g.N; q.NB = g.NB; q.t2_cap = g.t2_cap;
-    q.P = (uint32_t)g.P; q.cap = g.cap; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
+    q.N = g.N; q.NB = g.NB; q.t2_cap = g.t2_check;
+    q.P = (uint32_t)g.P; q.cap = g.cap; q.cap_check = g.cap_check; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
     q.tile_begin = tile_begin; q.tile_end = tile_end; q.slice_end_out = slice_end_out;

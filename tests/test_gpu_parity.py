@@ -292,3 +292,45 @@ def test_K24_full_parity(vx):
     assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
     assert plot.get_stats()["t2_records"] == 8386097        # tests/golden/match_counts.txt
     plot.free()
+
+
+# ------------------------------------------------------------------ overflow is an error, never a silent drop (A8)
+@pytest.mark.parametrize("flags", [0, 1])    # narrow; wide (stage 1 in rounds + compaction)
+def test_partition_overflow_raises(vx, flags):
+    key = vx_inputs.key_from_seed(5)
+    plot = vx.Plot(16, key, 12, flags=flags)            # 16 partitions of mean 4096, capacity 4608
+    plot.set_option(vx.VX_OPT_PARTITION_CAPACITY_LIMIT, 4000)
+    plot.build_table1()
+    with pytest.raises(vx.VxError, match="VX_ERR_OVERFLOW"):
+        plot.synchronize()
+    with pytest.raises(vx.VxError, match="VX_ERR_OVERFLOW"):
+        plot.read_tables(1)
+    # the same handle recovers once the capacity is back
+    plot.set_option(vx.VX_OPT_PARTITION_CAPACITY_LIMIT, plot.partition_capacity)
+    plot.build_table1()
+    plot.sort_match_table2()
+    assert plot.get_stats()["t1_records"] == 1 << 16
+    with pytest.raises(vx.VxError, match="VX_ERR_ARG"):
+        plot.set_option(vx.VX_OPT_PARTITION_CAPACITY_LIMIT, plot.partition_capacity + 1)
+    plot.free()
+
+
+def test_table2_overflow_raises(vx):
+    import torch
+    key = vx_inputs.key_from_seed(5)
+    plot = vx.Plot(16, key, 12)
+    plot.set_option(vx.VX_OPT_TABLE2_CAPACITY_LIMIT, 1000)   # |T2| ~ 2^16
+    plot.build_table1()
+    plot.sort_match_table2()
+    with pytest.raises(vx.VxError, match="VX_ERR_OVERFLOW"):
+        plot.synchronize()
+    # streamed egress reports it too
+    rec = torch.empty(1 << 20, dtype=torch.uint8, pin_memory=True)
+    plot.build_table1()
+    with pytest.raises(vx.VxError, match="VX_ERR_OVERFLOW"):
+        plot.sort_match_table2_to_host(torch.cuda.Stream(), rec.data_ptr(), rec.numel(), slices=4)
+    plot.set_option(vx.VX_OPT_TABLE2_CAPACITY_LIMIT, plot.t2_capacity)
+    plot.build_table1()
+    plot.sort_match_table2()
+    assert plot.get_stats()["t2_records"] > 60000
+    plot.free()
