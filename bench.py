@@ -41,9 +41,9 @@ ALU_OPS_PER_NONCE = 415            # xor / rotate / byte-swap lane-ops that need
 S2_BYTES_PER_NONCE = 12 + 12 + 8   # read record, write sorted record, write ~1 Table-2 record
 S1_BYTES_PER_NONCE = 12            # write the record once
 # DRAM bytes per nonce measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one
-# launch at K=29 / 2^29; profiles/r01_final.md) -- the same kernels and tile geometry at every K
-S1_DRAM_BYTES_PER_NONCE_NCU = 21.8
-S2_DRAM_BYTES_PER_NONCE_NCU = 40.4
+# launch at K=29 / 2^29; profiles/r01_final2.md) -- the same kernels and tile geometry at every K
+S1_DRAM_BYTES_PER_NONCE_NCU = 21.9
+S2_DRAM_BYTES_PER_NONCE_NCU = 40.3
 
 
 def measured_peaks():
@@ -319,7 +319,7 @@ def run_cuda(args):
               "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": S2_DRAM_BYTES_PER_NONCE_NCU * N, "ms": s2}
         r2["frac"] = r2["achieved"] / r2["peak"]
         dominant = dict(r1 if s1 >= s2 else r2)
-        dominant["traffic_source"] = ("ncu --set full at K=29 (profiles/r01_final.md): DRAM read+write bytes per "
+        dominant["traffic_source"] = ("ncu --set full at K=29 (profiles/r01_final2.md): DRAM read+write bytes per "
                                       "nonce of this kernel x 2^K")
         dominant["peak_source"] = peaks["source"] + (" (hbm_gbs, burst copy)" if dominant["bound"] == "hbm"
                                                      else " (sm_max_mhz x 148 SM x 4 SMSP x 16 ALU lanes; DESIGN.md)")
