@@ -297,9 +297,12 @@ def run_cuda(args):
 
     e2e_step()                      # warm the pinned path
     barrier()
+    e2e_each = []
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        e2e_step()
+        t1 = time.perf_counter()
+        e2e_step()                  # blocks until Table 2 is in host memory
+        e2e_each.append(time.perf_counter() - t1)
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
 
@@ -336,6 +339,7 @@ def run_cuda(args):
             "roofline": {k: dominant[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel", "peak_source", "traffic_source")},
             "e2e": {"value": world * N / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 32,
                     "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
+                    "seconds_each_rank0": [round(x, 4) for x in e2e_each],
                     "what": e2e_what},
             "gpu_launches": plot.launches_per_plot * args.steps,
             "clocks": clocks,

@@ -85,6 +85,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
         if (tmp_bytes > t2_bytes) t2_bytes = tmp_bytes;      // tiny K only
         g->off_cursor_tmp = o; o = align256(o + ((size_t)4 << g->pb_tmp));
     }
+    o = (o + ((size_t)2 << 20) - 1) & ~(((size_t)2 << 20) - 1);   // Table 2 on a 2 MB boundary: D2H copies of it run faster aligned
     g->off_t2_rec = o;    o = align256(o + t2_bytes);
     g->off_tmp = g->off_t2_rec;                              // scratch of stage 1, dead before stage 2
     if (g->wide) { g->off_t2_hi = o; o = align256(o + g->t2_cap); }
@@ -224,13 +225,19 @@ vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes)
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return fail_cuda(p, e, "cudaGetDevice (no CUDA device: there is no CPU fallback)");
-    cudaDeviceProp prop;
-    e = cudaGetDeviceProperties(&prop, dev);
-    if (e != cudaSuccess) return fail_cuda(p, e, "cudaGetDeviceProperties");
-    if (prop.major < 10) return fail(p, VX_ERR_CUDA, "libvx is built for sm_100a only");
-    p->num_sms = prop.multiProcessorCount;
-    e = vx_stage2_configure();
-    if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute(stage 2 shared memory)");
+    // attributes, not cudaGetDeviceProperties: that call takes 3-12 ms, and a plot is bound per key
+    int major = 0, sms = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaDeviceGetAttribute");
+    if (major < 10) return fail(p, VX_ERR_CUDA, "libvx is built for sm_100a only");
+    p->num_sms = sms;
+    static uint64_t configured = 0;                        // one bit per device ordinal < 64
+    if (dev >= 64 || !(configured & (1ull << dev))) {
+        e = vx_stage2_configure();
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute(stage 2 shared memory)");
+        if (dev < 64) configured |= 1ull << dev;
+    }
     p->ws = (uint8_t *)dev_workspace;
     p->ws_bytes = bytes;
     p->state = VX_BOUND;
