@@ -306,6 +306,18 @@ def run_cuda(args):
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
 
+    # ---- plot farm: two plots in flight (N=1 only; needs two workspaces + two pinned buffers) ----
+    # plot B is hashed, sorted and matched while plot A's Table 2 is still crossing PCIe
+    farm = None
+    free_b, _ = torch.cuda.mem_get_info()
+    if (world == 1 and streamed and args.e2e_inflight > 1
+            and free_b > plot.workspace_bytes + (2 << 30)):
+        try:
+            farm = run_farm(vx, torch, K, key, dev, plot, pinned_rec, pinned_off, rec_cap, nb,
+                            args.e2e_slices, max(8, e2e_steps))
+        except Exception as ex:                      # e.g. not enough pinned host memory
+            farm = {"unavailable": repr(ex)[:200]}
+
     # ---- max over ranks -------------------------------------------------------------------
     total_ms, e2e_s, s1, s2 = max_over_ranks(
         [total_ms, e2e_s, statistics.mean(s1_ms), statistics.mean(s2_ms)], world, dev)
@@ -340,7 +352,7 @@ def run_cuda(args):
             "e2e": {"value": world * N / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 32,
                     "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
                     "seconds_each_rank0": [round(x, 4) for x in e2e_each],
-                    "what": e2e_what},
+                    "what": e2e_what, "two_plots_in_flight": farm},
             "gpu_launches": plot.launches_per_plot * args.steps,
             "clocks": clocks,
         }
@@ -351,6 +363,48 @@ def run_cuda(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def run_farm(vx, torch, K, key, dev, plot, rec_a, off_a, rec_cap, nb, slices, steps_each):
+    """Two host threads, each plotting end to end into its own workspace and pinned buffers:
+    whole-plot throughput with the PCIe egress of one plot hidden behind the kernels of the other."""
+    ws_b = torch.empty(plot.workspace_bytes, dtype=torch.uint8, device=dev)
+    rec_b = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
+    off_b = torch.empty(nb + 1, dtype=torch.int64, pin_memory=True)
+    lanes = [(plot.workspace, rec_a, off_a), (ws_b, rec_b, off_b)]
+    streams = [(torch.cuda.Stream(), torch.cuda.Stream()) for _ in lanes]
+    errors = []
+
+    def worker(i, n):
+        try:
+            torch.cuda.set_device(dev)
+            ws, rec, off = lanes[i]
+            comp, copy = streams[i]
+            for _ in range(n):
+                p = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=ws)
+                p.build_table1(comp)
+                p.sort_match_table2_to_host(copy, rec.data_ptr(), rec_cap, off.data_ptr(), slices=slices, stream=comp)
+                p.free()
+        except Exception as ex:
+            errors.append(repr(ex))
+
+    def run(n):
+        th = [threading.Thread(target=worker, args=(i, n)) for i in range(len(lanes))]
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for t in th: t.start()
+        for t in th: t.join()
+        torch.cuda.synchronize()
+        return time.perf_counter() - t0
+
+    run(1)                                           # warm both lanes
+    dt = run(steps_each)
+    if errors:
+        raise RuntimeError(errors[0])
+    plots = len(lanes) * steps_each
+    return {"plots": plots, "seconds_per_plot": dt / plots, "value": plots * (1 << K) / dt, "unit": UNIT,
+            "what": "two host threads, one plot each in flight (own workspace, streams and pinned buffers): "
+                    "vx_build_table1 + vx_sort_match_table2_to_host back to back"}
 
 
 def main():
@@ -365,6 +419,8 @@ def main():
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=2)
     ap.add_argument("--e2e-chunks", dest="e2e_chunks", type=int, default=32)
     ap.add_argument("--e2e-slices", dest="e2e_slices", type=int, default=16)
+    ap.add_argument("--e2e-inflight", dest="e2e_inflight", type=int, default=2,
+                    help="2: also report end-to-end throughput with two plots in flight (N=1, K<=31)")
     ap.add_argument("--e2e-serial", dest="e2e_serial", action="store_true",
                     help="e2e with vx_read_tables after the plot instead of the streamed egress")
     ap.add_argument("--no-cpu-baseline", action="store_true")

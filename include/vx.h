@@ -195,8 +195,9 @@ vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uin
 vx_status vx_plot_layout(const vx_plot *p, uint32_t *wide, uint32_t *tile_log);
 
 /* Kernels one vx_build_table1 / vx_sort_match_table2 call launches (for the bench report's
- * gpu_launches): 2 + 1 in the narrow layout; the wide layout builds Table 1 in 4 rounds of
- * hash+scatter and compaction: 2 * 4 + 1 launches. */
+ * gpu_launches): 3 (clear, hash+scatter, partition scan) + 2 (clear, fused sort+match) in the narrow
+ * layout; the wide layout builds Table 1 in 4 rounds of hash+scatter and compaction
+ * (DESIGN.md "stage 1 in rounds"): 2 clears + 2 * 4 + 1 launches. */
 vx_status vx_plot_launches(const vx_plot *p, uint32_t *build_table1, uint32_t *sort_match_table2);
 
 const char *vx_last_error(const vx_plot *p); /* never NULL; includes cudaGetErrorString text */

@@ -360,16 +360,23 @@ static vx_status egress_common(vx_plot *p, void *compute_stream, void *copy_stre
     p->stream = (cudaStream_t)compute_stream;
     int soft = 0;
     char msg[256] = "";
+    VxCtrl ctrl;
+    memset(&ctrl, 0, sizeof ctrl);
     cudaError_t e = vx_egress_run(p->g, p->ws, p->force_exact, p->num_sms, p->stream, (cudaStream_t)copy_stream,
-                                  slices, host_records, records_capacity, host_offsets, ring, t2_records, &soft,
-                                  msg, sizeof msg);
+                                  slices, host_records, records_capacity, host_offsets, ring, t2_records, &ctrl,
+                                  &soft, msg, sizeof msg);
     if (e != cudaSuccess) return fail_cuda(p, e, "Table-2 egress");
     p->state = VX_MATCHED;
     p->t1_materialised = true;
     if (soft == 1) return fail(p, VX_ERR_RANGE, msg);
     if (soft == 2) return fail(p, VX_ERR_OVERFLOW, msg);
     if (soft == 3) return fail(p, VX_ERR_IO, msg);
-    return sync_and_check(p);
+    // both streams have drained inside vx_egress_run; the flags came back through the mailbox
+    if (ctrl.flags & VX_FLAG_PART_OVERFLOW)
+        return fail(p, VX_ERR_OVERFLOW, "a stage-1 partition exceeded its slack capacity");
+    if (ctrl.flags & VX_FLAG_T2_OVERFLOW)
+        return fail(p, VX_ERR_OVERFLOW, "Table 2 exceeded its capacity");
+    return VX_OK;
 }
 
 vx_status vx_sort_match_table2_to_host(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
@@ -497,7 +504,7 @@ vx_status vx_plot_launches(const vx_plot *p, uint32_t *build_table1, uint32_t *s
 {
     if (!p) return VX_ERR_ARG;
     if (build_table1) *build_table1 = vx_stage1_launches(p->g);
-    if (sort_match_table2) *sort_match_table2 = 1;
+    if (sort_match_table2) *sort_match_table2 = 2;   // clear + the fused kernel
     return VX_OK;
 }
 

@@ -27,6 +27,7 @@
 // cudaFreeHost was seen to block for 0.4 s behind other work, far too much for a per-call buffer.
 #include <mutex>
 #define VX_MAILBOXES 16
+#define VX_MAILBOX_WORDS (VX_EGRESS_MAX_SLICES + 8)   // slice ends + a copy of the control block
 static std::mutex g_mb_mutex;
 static unsigned long long *g_mb_host = nullptr, *g_mb_dev = nullptr;
 static uint32_t g_mb_busy = 0;
@@ -36,7 +37,7 @@ static int mailbox_acquire(unsigned long long **host, unsigned long long **dev, 
     std::lock_guard<std::mutex> lock(g_mb_mutex);
     *e = cudaSuccess;
     if (!g_mb_host) {
-        *e = cudaHostAlloc((void **)&g_mb_host, (size_t)VX_MAILBOXES * VX_EGRESS_MAX_SLICES * sizeof(unsigned long long),
+        *e = cudaHostAlloc((void **)&g_mb_host, (size_t)VX_MAILBOXES * VX_MAILBOX_WORDS * sizeof(unsigned long long),
                            cudaHostAllocMapped | cudaHostAllocPortable);
         if (*e == cudaSuccess) *e = cudaHostGetDevicePointer((void **)&g_mb_dev, g_mb_host, 0);
         if (*e != cudaSuccess) { if (g_mb_host) cudaFreeHost(g_mb_host); g_mb_host = nullptr; return -1; }
@@ -44,8 +45,8 @@ static int mailbox_acquire(unsigned long long **host, unsigned long long **dev, 
     for (int i = 0; i < VX_MAILBOXES; i++)
         if (!(g_mb_busy & (1u << i))) {
             g_mb_busy |= 1u << i;
-            *host = g_mb_host + (size_t)i * VX_EGRESS_MAX_SLICES;
-            *dev = g_mb_dev + (size_t)i * VX_EGRESS_MAX_SLICES;
+            *host = g_mb_host + (size_t)i * VX_MAILBOX_WORDS;
+            *dev = g_mb_dev + (size_t)i * VX_MAILBOX_WORDS;
             return i;
         }
     *e = cudaErrorMemoryAllocation;                     // more than VX_MAILBOXES egress calls in flight
@@ -57,6 +58,11 @@ static void mailbox_release(int i)
     std::lock_guard<std::mutex> lock(g_mb_mutex);
     if (i >= 0) g_mb_busy &= ~(1u << i);
 }
+
+// The control block (overflow flags, |Table 2|) goes to the host through the mailbox as well: a
+// cudaMemcpy of 32 bytes would queue on the copy engine behind ANOTHER plot's gigabytes of Table 2
+// and stall this plot's host thread until they have drained (two plots in flight, bench.py).
+__global__ void vx_k_publish_ctrl(const VxCtrl *__restrict__ ctrl, VxCtrl *__restrict__ out) { *out = *ctrl; }
 
 struct VxRing {
     uint8_t *base;        // pinned, caller-owned
@@ -108,8 +114,8 @@ static int ring_push(VxRing *r, const uint8_t *dev_src, size_t bytes, cudaStream
 // Shared driver.  host_records != NULL: memory sink.  ring != NULL: file sink.
 cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int num_sms, cudaStream_t compute,
                           cudaStream_t copy, uint32_t slices, uint8_t *host_records, size_t records_capacity,
-                          uint64_t *host_offsets, VxRing *ring, uint64_t *t2_records, int *soft_error,
-                          char *err, size_t errlen)
+                          uint64_t *host_offsets, VxRing *ring, uint64_t *t2_records, VxCtrl *ctrl_out,
+                          int *soft_error, char *err, size_t errlen)
 {
     *soft_error = 0;
     if (slices < 1) slices = 1;
@@ -130,6 +136,10 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
         const uint32_t t0 = (uint32_t)(P * s / slices), t1 = (uint32_t)(P * (s + 1) / slices);
         e = vx_launch_stage2(g, ws, true, force_exact, num_sms, compute, t0, t1, ends_dev + s);
         if (e == cudaSuccess) e = cudaEventRecord(ev[s], compute);
+    }
+    if (e == cudaSuccess) {
+        vx_k_publish_ctrl<<<1, 1, 0, compute>>>((const VxCtrl *)(ws + g.off_ctrl), (VxCtrl *)(ends_dev + VX_EGRESS_MAX_SLICES));
+        e = cudaGetLastError();
     }
     const uint8_t *t2_dev = ws + g.off_t2_rec;
     const uint8_t *off_dev = ws + g.off_t2_off;
@@ -173,6 +183,7 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
     e2 = cudaStreamSynchronize(compute);
     if (e == cudaSuccess) e = e2;
     if (t2_records) *t2_records = prev;
+    if (ctrl_out) memcpy(ctrl_out, ends + VX_EGRESS_MAX_SLICES, sizeof(VxCtrl));   // valid: compute has drained
     for (uint32_t i = 0; i < made; i++) cudaEventDestroy(ev[i]);
     mailbox_release(mailbox);
     return e;

@@ -79,6 +79,8 @@ void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_s
 // ---------------------------------------------------------------------------------- launches
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st);
 uint32_t vx_stage1_launches(const VxGeom &g);   // kernels vx_launch_stage1 enqueues
+// zero two regions and two words with a kernel (not a memset: see vx_k_clear)
+cudaError_t vx_launch_clear(cudaStream_t st, void *a, size_t bytes_a, void *b, size_t bytes_b, uint32_t *w0, uint32_t *w1);
 // sorts (and matches) the partitions [tile_begin, tile_end) -- (0, P) for the whole plot; slices must
 // be launched in ascending order on one stream.  slice_end_out (host-mapped, may be NULL) receives
 // the number of Table-2 records of the partitions < tile_end.
@@ -102,7 +104,7 @@ uint64_t vx_ring_written(const VxRing *r);
 void vx_ring_destroy(VxRing *r);
 cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int num_sms, cudaStream_t compute,
                           cudaStream_t copy, uint32_t slices, uint8_t *host_records, size_t records_capacity,
-                          uint64_t *host_offsets, VxRing *ring, uint64_t *t2_records, int *soft_error,
-                          char *err, size_t errlen);
+                          uint64_t *host_offsets, VxRing *ring, uint64_t *t2_records, VxCtrl *ctrl_out,
+                          int *soft_error, char *err, size_t errlen);
 cudaError_t vx_stage2_configure(void); // opt in to the large dynamic shared memory once
 size_t vx_stage2_smem_bytes(const VxGeom &g);

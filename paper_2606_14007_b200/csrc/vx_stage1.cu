@@ -64,7 +64,7 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint
 #define VX_CP_THREADS 256
 #define VX_CP_MAXSUB 4
 __global__ void __launch_bounds__(VX_CP_THREADS)
-vx_k_compact(const uint4 *__restrict__ tmp, const uint32_t *__restrict__ cursor_tmp, uint32_t cap_tmp,
+vx_k_compact(const uint4 *__restrict__ tmp, uint32_t *__restrict__ cursor_tmp, uint32_t cap_tmp,
              uint32_t pb, uint32_t d, uint32_t nlo_bits, uint32_t cap, uint32_t cap_check,
              unsigned long long *__restrict__ part_a, uint16_t *__restrict__ part_b,
              uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
@@ -106,6 +106,30 @@ vx_k_compact(const uint4 *__restrict__ tmp, const uint32_t *__restrict__ cursor_
     if (over) atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
     __syncthreads();
     if (tid < nsub) cursor[(p << d) + tid] = s_base[tid] + s_cnt[tid];   // counts every claim, like stage 1's atomics
+    if (tid == 0) cursor_tmp[p] = 0u;                   // ready for the next round (read above, before the first barrier)
+}
+
+// Zeroes up to two regions (16-byte granules; every workspace region is 256-byte aligned and padded)
+// and up to two single words.  A kernel rather than cudaMemsetAsync: a memset may be handed to a copy
+// engine, where it queues behind another plot's gigabyte-sized Table-2 copies (vx_egress.cu) and
+// holds this plot's kernels back until they drain.
+__global__ void __launch_bounds__(256)
+vx_k_clear(uint4 *__restrict__ a, size_t na, uint4 *__restrict__ b, size_t nb, uint32_t *w0, uint32_t *w1)
+{
+    const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x, step = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = i0; i < na; i += step) a[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (size_t i = i0; i < nb; i += step) b[i] = make_uint4(0u, 0u, 0u, 0u);
+    if (i0 == 0) { if (w0) *w0 = 0u; if (w1) *w1 = 0u; }
+}
+
+cudaError_t vx_launch_clear(cudaStream_t st, void *a, size_t bytes_a, void *b, size_t bytes_b, uint32_t *w0, uint32_t *w1)
+{
+    const size_t na = (bytes_a + 15) / 16, nb = (bytes_b + 15) / 16;
+    size_t grid = ((na > nb ? na : nb) + 255) / 256;
+    if (grid < 1) grid = 1;
+    if (grid > 148 * 8) grid = 148 * 8;
+    vx_k_clear<<<(unsigned)grid, 256, 0, st>>>((uint4 *)a, na, (uint4 *)b, nb, w0, w1);
+    return cudaGetLastError();
 }
 
 // Exclusive prefix sum of the clamped partition counts: part_base[p] = number of records in
@@ -202,16 +226,19 @@ vx_k_hash_sink(const __grid_constant__ VxHashConst hc, uint64_t count, uint64_t 
 }
 
 // ----------------------------------------------------------------------------- launches
-uint32_t vx_stage1_launches(const VxGeom &g) { return g.wide ? 2u * g.rounds + 1u : 2u; }
+uint32_t vx_stage1_launches(const VxGeom &g) { return g.wide ? 2u * g.rounds + 3u : 3u; }   // + the clears
 
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st)
 {
     VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
     uint32_t *cursor = (uint32_t *)(ws + g.off_cursor);
-    cudaError_t e = cudaMemsetAsync(ctrl, 0, sizeof(VxCtrl), st);
+    // ctrl + cursors (the wide layout's scratch cursors follow the final ones in the workspace plan)
+    cudaError_t e = vx_launch_clear(st, ctrl, sizeof(VxCtrl), cursor, g.P * sizeof(uint32_t), nullptr, nullptr);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(cursor, 0, g.P * sizeof(uint32_t), st);
-    if (e != cudaSuccess) return e;
+    if (g.wide) {
+        e = vx_launch_clear(st, ws + g.off_cursor_tmp, sizeof(uint32_t) << g.pb_tmp, nullptr, 0, nullptr, nullptr);
+        if (e != cudaSuccess) return e;
+    }
     const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
     uint4 *part = (uint4 *)(ws + g.off_part);
     uint16_t *part_b = (uint16_t *)(ws + g.off_part_b);
@@ -224,8 +251,6 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
         const uint64_t slice = 1ull << g.round_log;
         const uint64_t grid = (slice + per_cta - 1) / per_cta;
         for (uint32_t r = 0; r < g.rounds; r++) {
-            e = cudaMemsetAsync(cursor_tmp, 0, sizeof(uint32_t) << g.pb_tmp, st);
-            if (e != cudaSuccess) return e;
             if (g.nonce_size == 5)
                 vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
                     hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);

@@ -625,14 +625,11 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
     if (tile_end > g.P) tile_end = (uint32_t)g.P;
     if (tile_begin >= tile_end) return cudaErrorInvalidValue;
-    cudaError_t e = cudaMemsetAsync(&ctrl->ticket, 0, sizeof(uint32_t), st);
+    // ticket; for the first (or only) slice of the plot also the largest-bucket word and the look-back state
+    const bool first = tile_begin == 0;
+    cudaError_t e = vx_launch_clear(st, first ? ws + g.off_status : nullptr, first ? g.P * sizeof(unsigned long long) : 0,
+                                    nullptr, 0, &ctrl->ticket, first ? &ctrl->max_bucket : nullptr);
     if (e != cudaSuccess) return e;
-    if (tile_begin == 0) {                              // first (or only) slice of the plot
-        e = cudaMemsetAsync(&ctrl->max_bucket, 0, sizeof(uint32_t), st);
-        if (e != cudaSuccess) return e;
-        e = cudaMemsetAsync(ws + g.off_status, 0, g.P * sizeof(unsigned long long), st);
-        if (e != cudaSuccess) return e;
-    }
     VxS2Params q;
     q.part = (uint4 *)(ws + g.off_part);
     q.cursor = (const uint32_t *)(ws + g.off_cursor);

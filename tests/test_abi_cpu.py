@@ -59,9 +59,9 @@ def test_create_validates_arguments():
     assert L.vx_plot_create(33, key, ctypes.byref(h)) == 0 and h.value   # 5-byte nonces, wide layout
     ns = ctypes.c_uint32()
     assert L.vx_plot_info(h, None, None, ctypes.byref(ns), None, None, None) == 0 and ns.value == 5
-    # wide layout: Table 1 is built in 4 rounds of hash+scatter and compaction, + the partition scan
+    # wide layout: 2 clears, 4 rounds of hash+scatter and compaction, the partition scan
     l1, l2 = ctypes.c_uint32(), ctypes.c_uint32()
-    assert L.vx_plot_launches(h, ctypes.byref(l1), ctypes.byref(l2)) == 0 and (l1.value, l2.value) == (9, 1)
+    assert L.vx_plot_launches(h, ctypes.byref(l1), ctypes.byref(l2)) == 0 and (l1.value, l2.value) == (11, 2)
     # streamed egress: not before vx_build_table1 (and never for 5-byte nonces)
     assert L.vx_sort_match_table2_to_host(h, None, ctypes.c_void_p(8), 4, ctypes.c_void_p(8), 0, None, None) == -2
     assert L.vx_sort_match_table2_to_file(h, None, ctypes.c_void_p(8), 4, -1, None, 0, None) == -1
@@ -72,7 +72,7 @@ def test_create_validates_arguments():
     t2 = ctypes.c_uint64()
     assert L.vx_plot_info(h, *[ctypes.byref(x) for x in info], ctypes.byref(t2)) == 0
     assert [x.value for x in info[:4]] == [20, 24, 4, 8]
-    assert L.vx_plot_launches(h, ctypes.byref(l1), ctypes.byref(l2)) == 0 and (l1.value, l2.value) == (2, 1)
+    assert L.vx_plot_launches(h, ctypes.byref(l1), ctypes.byref(l2)) == 0 and (l1.value, l2.value) == (3, 2)
     # out-of-order calls
     assert L.vx_build_table1(h, None) == -2
     assert L.vx_sort_match_table2(h, None) == -2
