@@ -254,13 +254,17 @@ def run_cuda(args):
     nb = 1 << BUCKET_BITS
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     d2h = 0
-    streamed = plot.nonce_size == 4 and not args.e2e_serial
+    streamed = not args.e2e_serial
     if streamed:
         # vx_sort_match_table2_to_host: stage 2 in slices, each finished slice copied
         # on a second stream straight into place in one pinned buffer while later slices are matched
-        copy_stream = torch.cuda.Stream()
         rec_cap = plot.rec2_bytes * plot.t2_capacity
-        pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
+        try:
+            pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)   # K=33: 86 GB
+        except RuntimeError:
+            streamed = False                         # not enough pinnable host memory: ranged reads
+    if streamed:
+        copy_stream = torch.cuda.Stream()
         pinned_off = torch.empty(nb + 1, dtype=torch.int64, pin_memory=True)
         e2e_what = ("vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2_to_host(Table 2 + offsets into "
                     f"pinned host memory on a second stream, {args.e2e_slices} slices overlapped with the matching)")
@@ -273,8 +277,7 @@ def run_cuda(args):
                                                slices=args.e2e_slices, stream=stream) + (nb + 1) * 8
             p2.free()
     else:
-        # 5-byte nonces (K = 33): Table 2 is resident in a packed form; vx_read_tables converts and
-        # copies it range by range after the plot
+        # vx_read_tables copies (5-byte nonces: converts and copies) Table 2 range by range after the plot
         chunks = args.e2e_chunks
         per = nb // chunks
         rec_cap = int(1.25 * plot.rec2_bytes * (N // chunks)) + (1 << 20)

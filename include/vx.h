@@ -108,7 +108,8 @@ vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream);
  * compute_stream (1..256; clamped), and the Table-2 records and CSR offsets of each finished slice
  * are copied on copy_stream (a different stream) while the later slices are still being matched.
  * Both BLOCK until everything has arrived and report device-raised errors like vx_synchronize.
- * K <= 32 only (VX_ERR_UNSUPPORTED for 5-byte nonces, whose Table 2 is resident in a packed form).
+ * With 5-byte nonces (K = 33) Table 2 is resident in a packed form: each chunk is first converted to
+ * the external format in the workspace's staging area (a kernel on copy_stream), then copied.
  *
  * _to_host: host_records (HOST, caller-owned, pinned for the copies to overlap; records_capacity
  *   bytes, VX_ERR_RANGE if too small) receives all of Table 2 in the external format, bucket-major;

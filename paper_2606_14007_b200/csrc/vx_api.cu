@@ -354,8 +354,6 @@ static vx_status egress_common(vx_plot *p, void *compute_stream, void *copy_stre
                                VxRing *ring, uint64_t *t2_records)
 {
     if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "Table-2 egress before vx_build_table1");
-    if (p->g.nonce_size > 4)
-        return fail(p, VX_ERR_UNSUPPORTED, "streamed egress needs Table 2 resident in the external format (K <= 32)");
     if (compute_stream == copy_stream) return fail(p, VX_ERR_ARG, "compute and copy streams must differ");
     p->stream = (cudaStream_t)compute_stream;
     int soft = 0;

@@ -143,7 +143,26 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
     }
     const uint8_t *t2_dev = ws + g.off_t2_rec;
     const uint8_t *off_dev = ws + g.off_t2_off;
-    const size_t rb = 8;                                  // narrow Table-2 records are resident in the external format
+    // 4-byte nonces: Table 2 is resident in the external format and is copied straight out.  5-byte
+    // nonces (K = 33): it is resident packed (uint2 + a byte of high bits), so every chunk first goes
+    // through vx_k_export_t2 into the workspace's staging area, on the copy stream, chunk by chunk.
+    // The staging area is used as two halves: the conversion of chunk k + 1 (on a stream of its own)
+    // runs while chunk k is crossing PCIe.
+    const bool packed = g.nonce_size > 4;
+    const size_t rb = g.rec2_bytes;
+    const size_t half = (g.stage_bytes / 2) & ~(size_t)255;
+    uint64_t chunk_rec = half / rb;                       // packed: records per staging half,
+    if (chunk_rec >= (1u << 20)) chunk_rec &= ~(uint64_t)((1u << 20) - 1);   // a multiple of 2 MB in bytes
+    cudaStream_t xs = nullptr;                            // packed: the conversion kernels' stream
+    cudaEvent_t exported[2] = {nullptr, nullptr}, drained[2] = {nullptr, nullptr};
+    uint64_t chunk_no = 0;
+    if (packed && e == cudaSuccess) {
+        e = cudaStreamCreateWithFlags(&xs, cudaStreamNonBlocking);
+        for (int h = 0; h < 2 && e == cudaSuccess; h++) {
+            e = cudaEventCreateWithFlags(&exported[h], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&drained[h], cudaEventDisableTiming);
+        }
+    }
     uint64_t prev = 0, copied = 0;                        // records accounted for / bytes already enqueued
     for (uint32_t s = 0; e == cudaSuccess && s < slices && !*soft_error; s++) {
         e = cudaEventSynchronize(ev[s]);                  // slice s is sorted, matched and emitted
@@ -152,8 +171,31 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
         const uint32_t t0 = (uint32_t)(P * s / slices), t1 = (uint32_t)(P * (s + 1) / slices);
         const uint64_t b0 = (uint64_t)t0 << g.fb, b1 = (uint64_t)t1 << g.fb;
         if (cur < prev || cur > g.t2_check) { snprintf(err, errlen, "Table 2 exceeded its capacity"); *soft_error = 2; break; }
-        if (host_records) {
-            if (cur * rb > records_capacity) { snprintf(err, errlen, "records_capacity too small"); *soft_error = 1; break; }
+        if (host_records && cur * rb > records_capacity) { snprintf(err, errlen, "records_capacity too small"); *soft_error = 1; break; }
+        if (packed) {
+            // whole staging chunks only, except behind the last slice
+            const uint64_t avail = s + 1 == slices ? cur : cur - cur % chunk_rec;
+            uint64_t done = copied / rb;
+            while (e == cudaSuccess && done < avail && !*soft_error) {
+                const uint64_t n = avail - done < chunk_rec ? avail - done : chunk_rec;
+                const int h = (int)(chunk_no & 1);
+                const size_t so = h ? half : 0;
+                if (chunk_no >= 2) e = cudaStreamWaitEvent(xs, drained[h], 0);   // the half is free again
+                if (e == cudaSuccess) e = vx_launch_export_t2(g, ws, done, n, xs, so);
+                if (e == cudaSuccess) e = cudaEventRecord(exported[h], xs);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, exported[h], 0);
+                if (e != cudaSuccess) break;
+                if (host_records)
+                    e = cudaMemcpyAsync(host_records + done * rb, ws + g.off_stage + so, n * rb, cudaMemcpyDeviceToHost, copy);
+                else if (ring_push(ring, ws + g.off_stage + so, n * rb, copy, err, errlen))
+                    *soft_error = 3;
+                if (e == cudaSuccess) e = cudaEventRecord(drained[h], copy);
+                done += n;
+                chunk_no++;
+            }
+            copied = done * rb;
+            if (*soft_error) break;
+        } else if (host_records) {
             // copies begin and end on 2 MB boundaries of the record stream (the unaligned tail of a slice
             // travels with the next one) and are at most 1 GB long: measured on this box, D2H into a
             // large pinned buffer runs at 55 GB/s that way, 53.5 GB/s with unaligned ends and
@@ -182,6 +224,8 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
     if (e == cudaSuccess) e = e2;
     e2 = cudaStreamSynchronize(compute);
     if (e == cudaSuccess) e = e2;
+    if (xs) { cudaStreamSynchronize(xs); cudaStreamDestroy(xs); }
+    for (int h = 0; h < 2; h++) { if (exported[h]) cudaEventDestroy(exported[h]); if (drained[h]) cudaEventDestroy(drained[h]); }
     if (t2_records) *t2_records = prev;
     if (ctrl_out) memcpy(ctrl_out, ends + VX_EGRESS_MAX_SLICES, sizeof(VxCtrl));   // valid: compute has drained
     for (uint32_t i = 0; i < made; i++) cudaEventDestroy(ev[i]);

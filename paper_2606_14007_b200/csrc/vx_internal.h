@@ -90,7 +90,8 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
 // external-format Table-1 records [first, first + count) of the CSR numbering -> ws + off_stage
 cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
 // wide, NONCE_SIZE = 5: external 10-byte Table-2 records [first, first + count) -> ws + off_stage
-cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
+cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st,
+                                size_t stage_offset = 0);   // ... + stage_offset
 cudaError_t vx_launch_hash_range(const VxGeom &g, const VxHashConst &hc, uint64_t nonce_begin,
                                  uint64_t count, uint64_t *dev_hashes, cudaStream_t st);
 cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t count,

@@ -583,13 +583,13 @@ cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, ui
 }
 
 cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count,
-                                cudaStream_t st)
+                                cudaStream_t st, size_t stage_offset)
 {
     if (count == 0) return cudaSuccess;
     uint64_t grid = (count + 255) / 256;
     if (grid > 148 * 16) grid = 148 * 16;
     vx_k_export_t2<<<(unsigned)grid, 256, 0, st>>>((const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi,
-                                                   first, count, ws + g.off_stage);
+                                                   first, count, ws + g.off_stage + stage_offset);
     return cudaGetLastError();
 }
 

@@ -105,13 +105,3 @@ def test_streamed_table2_to_file(vx, tmp_path, K, B, seed, slices, ring_chunks):
     tr = data[-32:]
     assert bytes(tr[:8]) == b"VXT2\0\0\0\1"
     assert list(tr[8:24].view(np.uint32)) == [K, B, 4, 0] and int(tr[24:].view(np.uint64)[0]) == m
-
-
-def test_streamed_egress_unsupported_for_5_byte_nonces(vx):
-    L = vx.load_library()
-    import ctypes
-    h = ctypes.c_void_p()
-    assert L.vx_plot_create(33, vx_inputs.key_from_seed(33), ctypes.byref(h)) == 0
-    # not bound: state error comes first; the layout check needs no device memory either way
-    assert L.vx_sort_match_table2_to_host(h, None, ctypes.c_void_p(1), 4, ctypes.c_void_p(1), 0, None, None) in (-2, -7)
-    L.vx_free(h)

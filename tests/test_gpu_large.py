@@ -293,3 +293,61 @@ def test_K33_full_size_samples_and_properties(vx):
         assert int(seen.sum()) == R, "some nonce is missing from Table 1 (or appears twice)"
         del seen
     plot.free()
+
+
+def test_K33_streamed_egress_of_packed_table2(vx):
+    """SURVEY 8(f1) at K=33: Table 2 is resident packed (uint2 + a byte of high nonce bits), so the
+    egress pipeline converts it chunk by chunk in the staging area before the copy.  86 GB stream
+    to pinned host memory, checked against vx_read_tables on sampled bucket ranges, among them the
+    ranges that straddle the first staging-chunk boundaries and the slice boundaries; then the file
+    sink into /dev/null (byte count)."""
+    import os
+    import torch
+    K, B = 33, 24
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    need = vx.workspace_bytes(K)
+    if free < need + (6 << 30):
+        pytest.skip(f"needs {need / 1e9:.0f} GB + 6 GB of device memory, {free / 1e9:.0f} GB free")
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    cap = plot.rec2_bytes * plot.t2_capacity
+    try:
+        rec = torch.empty(cap, dtype=torch.uint8, pin_memory=True)
+    except RuntimeError as ex:
+        plot.free()
+        pytest.skip(f"cannot pin {cap / 1e9:.0f} GB of host memory: {ex}")
+    off = torch.empty((1 << B) + 1, dtype=torch.int64, pin_memory=True)
+    off.fill_(-1)
+    copy = torch.cuda.Stream()
+    slices = 16
+    plot.build_table1()
+    got = plot.sort_match_table2_to_host(copy, rec.data_ptr(), cap, off.data_ptr(), slices=slices)
+    stats = plot.get_stats()
+    assert got == 10 * stats["t2_records"]
+    o = off.numpy()
+    assert o[0] == 0 and o[-1] == stats["t2_records"] and bool((np.diff(o) >= 0).all())
+    r = rec.numpy()
+    NB = 1 << B
+    chunk_rec = ((32 << 20) // 10) & ~((1 << 20) - 1)        # records per staging half (vx_egress.cu)
+    starts = [0, NB - 8]
+    starts += [max(0, int(np.searchsorted(o, k * chunk_rec)) - 4) for k in (1, 2, 3, 700)]
+    starts += [NB * s // slices - 4 for s in (1, 2, 9, 15)]
+    starts += [int(x) for x in np.random.default_rng(7).integers(0, NB - 8, 6)]
+    checked = 0
+    for b0 in starts:
+        offs, raw = plot.read_tables(2, b0, b0 + 8)
+        assert np.array_equal(offs, (o[b0:b0 + 9] - o[b0]).astype(np.uint64))
+        assert np.array_equal(raw, r[10 * o[b0]: 10 * o[b0 + 8]])
+        checked += len(raw) // 10
+    assert checked > 50000
+    # file sink, packed path: records, offsets, trailer -- only the byte count can be checked here
+    ring = torch.empty(64 << 20, dtype=torch.uint8, pin_memory=True)
+    fd = os.open("/dev/null", os.O_WRONLY)
+    try:
+        plot.build_table1()
+        nbytes = plot.sort_match_table2_to_file(copy, fd, ring.data_ptr(), ring.numel(), slices=slices)
+    finally:
+        os.close(fd)
+    assert nbytes == 10 * stats["t2_records"] + 8 * (NB + 1) + 32
+    plot.free()
