@@ -41,7 +41,7 @@ ALU_OPS_PER_NONCE = 415            # xor / rotate / byte-swap lane-ops that need
 S2_BYTES_PER_NONCE = 12 + 12 + 8   # read record, write sorted record, write ~1 Table-2 record
 S1_BYTES_PER_NONCE = 12            # write the record once
 # DRAM bytes per nonce measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one
-# launch at K=29 / 2^29; profiles/r01_final2.md) -- the same kernels and tile geometry at every K
+# launch at K=29 / 2^29; profiles/r01_final3.md) -- the same kernels and tile geometry at every K
 S1_DRAM_BYTES_PER_NONCE_NCU = 21.9
 S2_DRAM_BYTES_PER_NONCE_NCU = 40.3
 
@@ -260,8 +260,13 @@ def run_cuda(args):
         # on a second stream straight into place in one pinned buffer while later slices are matched
         rec_cap = plot.rec2_bytes * plot.t2_capacity
         try:
-            pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)   # K=33: 86 GB
-        except RuntimeError:
+            # every local rank pins a whole Table 2 (K=31: 17 GB, K=33: 86 GB): only with room to spare
+            import psutil
+            local_world = int(os.environ.get("LOCAL_WORLD_SIZE", str(world)))
+            if psutil.virtual_memory().available < 1.5 * rec_cap * local_world + (8 << 30):
+                raise RuntimeError("host memory")
+            pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
+        except (RuntimeError, ImportError):
             streamed = False                         # not enough pinnable host memory: ranged reads
     if streamed:
         copy_stream = torch.cuda.Stream()
@@ -313,7 +318,13 @@ def run_cuda(args):
     # plot B is hashed, sorted and matched while plot A's Table 2 is still crossing PCIe
     farm = None
     free_b, _ = torch.cuda.mem_get_info()
-    if (world == 1 and streamed and args.e2e_inflight > 1
+    host_ok = False
+    try:
+        import psutil
+        host_ok = psutil.virtual_memory().available > 1.5 * plot.rec2_bytes * plot.t2_capacity + (8 << 30)
+    except ImportError:
+        pass
+    if (world == 1 and streamed and host_ok and args.e2e_inflight > 1
             and free_b > plot.workspace_bytes + (2 << 30)):
         try:
             farm = run_farm(vx, torch, K, key, dev, plot, pinned_rec, pinned_off, rec_cap, nb,
@@ -337,7 +348,7 @@ def run_cuda(args):
               "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": S2_DRAM_BYTES_PER_NONCE_NCU * N, "ms": s2}
         r2["frac"] = r2["achieved"] / r2["peak"]
         dominant = dict(r1 if s1 >= s2 else r2)
-        dominant["traffic_source"] = ("ncu --set full at K=29 (profiles/r01_final2.md): DRAM read+write bytes per "
+        dominant["traffic_source"] = ("ncu --set full at K=29 (profiles/r01_final3.md): DRAM read+write bytes per "
                                       "nonce of this kernel x 2^K")
         dominant["peak_source"] = peaks["source"] + (" (hbm_gbs, burst copy)" if dominant["bound"] == "hbm"
                                                      else " (sm_max_mhz x 148 SM x 4 SMSP x 16 ALU lanes; DESIGN.md)")
