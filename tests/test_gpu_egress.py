@@ -105,3 +105,44 @@ def test_streamed_table2_to_file(vx, tmp_path, K, B, seed, slices, ring_chunks):
     tr = data[-32:]
     assert bytes(tr[:8]) == b"VXT2\0\0\0\1"
     assert list(tr[8:24].view(np.uint32)) == [K, B, 4, 0] and int(tr[24:].view(np.uint64)[0]) == m
+
+
+def test_two_plots_in_flight_from_two_threads(vx):
+    """bench.py's e2e.two_plots_in_flight path: two host threads, each with its own plot, workspace,
+    streams and pinned buffers, plotting end to end at the same time (shared: the library's mailbox
+    pool and the copy engines).  Every plot of both threads must be the oracle's."""
+    import threading
+    import torch
+    cases = [(20, 24, 1), (19, 12, 9)]
+    want = [oracle_tables(K, vx_inputs.key_from_seed(seed), B) for K, B, seed in cases]
+    errors = []
+
+    def worker(i):
+        try:
+            K, B, seed = cases[i]
+            o_off, o_non, o_has, o_t2o, o_n1, o_n2 = want[i]
+            key = vx_inputs.key_from_seed(seed)
+            comp, copy = torch.cuda.Stream(), torch.cuda.Stream()
+            rec = pinned(8 * len(o_n1) + 64)
+            off = torch.empty((1 << B) + 1, dtype=torch.int64, pin_memory=True)
+            ws = None
+            for rep in range(4):
+                plot = vx.Plot(K, key, B, workspace=ws)
+                ws = plot.workspace
+                rec.fill_(0); off.fill_(-1)
+                plot.build_table1(comp)
+                got = plot.sort_match_table2_to_host(copy, rec.data_ptr(), rec.numel(), off.data_ptr(),
+                                                     slices=5 + rep, stream=comp)
+                assert got == 8 * len(o_n1)
+                off2 = off.numpy().view(np.uint64)
+                assert np.array_equal(off2, o_t2o)
+                g1, g2 = canon_t2(off2, *decode_t2(rec.numpy()[:got], 4))
+                assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+                plot.free()
+        except BaseException as ex:   # noqa: BLE001 - reported by the main thread
+            errors.append(f"thread {i}: {ex!r}")
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in threads: t.start()
+    for t in threads: t.join()
+    assert not errors, errors
