@@ -432,7 +432,7 @@ def main():
     ap.add_argument("--ref-K", dest="ref_K", type=int, default=22, help="oracle sample size per --impl reference step")
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=2)
     ap.add_argument("--e2e-chunks", dest="e2e_chunks", type=int, default=32)
-    ap.add_argument("--e2e-slices", dest="e2e_slices", type=int, default=16)
+    ap.add_argument("--e2e-slices", dest="e2e_slices", type=int, default=64)
     ap.add_argument("--e2e-inflight", dest="e2e_inflight", type=int, default=2,
                     help="2: also report end-to-end throughput with two plots in flight (N=1, K<=31)")
     ap.add_argument("--e2e-serial", dest="e2e_serial", action="store_true",
