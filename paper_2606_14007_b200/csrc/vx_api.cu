@@ -147,6 +147,8 @@ static vx_status sync_and_check(vx_plot *p)
         VxCtrl c;
         e = cudaMemcpy(&c, p->ws + p->g.off_ctrl, sizeof c, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(ctrl)");
+        if (c.flags & VX_FLAG_BOUNDS)
+            return fail(p, VX_ERR_CUDA, "internal bounds check failed (VX_DEBUG_BOUNDS build)");
         if (c.flags & VX_FLAG_PART_OVERFLOW)
             return fail(p, VX_ERR_OVERFLOW, "a stage-1 partition exceeded its slack capacity");
         if (c.flags & VX_FLAG_T2_OVERFLOW)
@@ -370,6 +372,8 @@ static vx_status egress_common(vx_plot *p, void *compute_stream, void *copy_stre
     if (soft == 2) return fail(p, VX_ERR_OVERFLOW, msg);
     if (soft == 3) return fail(p, VX_ERR_IO, msg);
     // both streams have drained inside vx_egress_run; the flags came back through the mailbox
+    if (ctrl.flags & VX_FLAG_BOUNDS)
+        return fail(p, VX_ERR_CUDA, "internal bounds check failed (VX_DEBUG_BOUNDS build)");
     if (ctrl.flags & VX_FLAG_PART_OVERFLOW)
         return fail(p, VX_ERR_OVERFLOW, "a stage-1 partition exceeded its slack capacity");
     if (ctrl.flags & VX_FLAG_T2_OVERFLOW)

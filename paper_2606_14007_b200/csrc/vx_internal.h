@@ -69,6 +69,19 @@ struct VxCtrl {
 };
 #define VX_FLAG_PART_OVERFLOW 1u
 #define VX_FLAG_T2_OVERFLOW 2u
+#define VX_FLAG_BOUNDS 4u        // a VX_CHECK failed (debug build only)
+// Index checks of our own (compute-sanitizer is not available on the GPU pool): built with
+// -DVX_DEBUG_BOUNDS=1 (VX_NVCC_EXTRA, paper_2606_14007_b200/build.py) every shared- and global-memory
+// index of the kernels is checked against its array and a failure surfaces as VX_ERR_CUDA
+// "internal bounds check failed" at the next synchronising call.  Empty in the product build.
+#ifndef VX_DEBUG_BOUNDS
+#define VX_DEBUG_BOUNDS 0
+#endif
+#if VX_DEBUG_BOUNDS
+#define VX_CHECK(ctrl, cond) do { if (!(cond)) atomicOr(&(ctrl)->flags, VX_FLAG_BOUNDS); } while (0)
+#else
+#define VX_CHECK(ctrl, cond) do { } while (0)
+#endif
 
 // returns false if (K, B) is not a supported geometry
 bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles);

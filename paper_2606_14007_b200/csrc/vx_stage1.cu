@@ -38,8 +38,10 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint
         const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
         if (n < N) {
             const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
+            VX_CHECK(ctrl, pb == 0 || p < (1u << pb));
             const uint32_t slot = atomicAdd(&cursor[p], 1u);
             if (slot < cap_check) {                     // = cap, unless a test lowered it
+                VX_CHECK(ctrl, slot < cap);
                 // one 16-byte store per record: scattered stores are bound by requests, not bytes
                 part[(uint64_t)p * cap + slot] =
                     make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)n, (uint32_t)(n >> 32));
@@ -94,8 +96,10 @@ vx_k_compact(const uint4 *__restrict__ tmp, uint32_t *__restrict__ cursor_tmp, u
         off = __shfl_sync(0xffffffffu, off, leader);
         if (valid) {
             const uint32_t slot = s_base[s] + off + __popc(peers & ((1u << lane) - 1u));
+            VX_CHECK(ctrl, s < nsub && nsub <= VX_CP_MAXSUB);
             if (slot < cap_check) {
                 const size_t at = (size_t)((p << d) + s) * cap + slot;
+                VX_CHECK(ctrl, slot < cap && ((p << d) + s) < (1u << pb));
                 part_a[at] = (H << pb) | (n >> nlo_bits);
                 part_b[at] = (uint16_t)(n & ((1u << nlo_bits) - 1u));
             } else {

@@ -218,6 +218,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t i = it * THREADS + tid;
                     const uint32_t e0 = E[i];
                     const uint32_t c = E[i + 1] - e0;
+                    VX_CHECK(q.ctrl, i + 1 <= (uint32_t)CAPA && e0 + c <= M && (c == 0 || i + c < cnt) && base2 + e0 + c <= q.t2_cap);
                     const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
                     if (cmax) {
                         if constexpr (WIDE) {
@@ -293,6 +294,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 const uint32_t idx = it * THREADS + tid;
+                VX_CHECK(q.ctrl, cnt <= (uint32_t)CAPA && cnt <= q.cap && vx_bin<VX_NBINS>(key[it], sh) < VX_NBINS);
                 if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin<VX_NBINS>(key[it], sh)], 1u);
             }
             if (pending) {                              // the previous tile of this CTA: look-back + H
@@ -321,6 +323,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t idx = it * THREADS + tid;
                     if (idx < cnt) {
                         const uint32_t pos = bins[vx_bin<VX_NBINS>(key[it], sh)] + sn[it];
+                        VX_CHECK(q.ctrl, pos < cnt);
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
                         sub[pos] = vx_subkey(key[it], sh);
@@ -340,6 +343,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t b = vx_bin<VX_NBINS>(k, sh);
                     const uint32_t s = bins[b];
                     uint32_t n = bins[b + 1] - s;
+                    VX_CHECK(q.ctrl, b < VX_NBINS && (i >= cnt || (s <= i && i < s + n && s + n <= cnt)));
                     if (i >= cnt || n == 1) n = 0;      // alone in its bin: stays
                     const uint32_t nm = __reduce_max_sync(VX_FULL, n);
                     uint32_t rank = 0;
@@ -378,6 +382,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 if (it * THREADS + wbase < cnt) {
                     if (sn[it] >> 16) {
                         const uint32_t pos = sn[it] & 0xffffu;
+                        VX_CHECK(q.ctrl, pos < cnt);
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
                     }
@@ -427,6 +432,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             }
                         }
                     }
+                    VX_CHECK(q.ctrl, i < (uint32_t)CAPA && (c == 0 || i + c < cnt));
                     E[i] = c;
                 }
             }
@@ -475,6 +481,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         const unsigned long long gb0 = (unsigned long long)tile << q.fb;
         for (uint32_t bl = tid; bl < nb_local; bl += THREADS) {
             const uint32_t s = bucket_start(bl), e = bucket_start(bl + 1);
+            VX_CHECK(q.ctrl, s <= e && e <= cnt && gb0 + bl < q.NB && (!defer || bl < VX_DEFER_MAXB));
             cta_max_bucket = max(cta_max_bucket, e - s);
             q.t1_off[gb0 + bl] = base1 + s;
             if (defer) s_e2[bl] = E[s];
