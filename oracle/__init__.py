@@ -71,6 +71,13 @@ def lib() -> ctypes.CDLL:
         L.vxo_table1_slice.restype = U64
         L.vxo_table1_slice.argtypes = [ctypes.c_int, ctypes.c_char_p, ctypes.c_int, U64, U64,
                                        _p64, _p64, _p64, U64]
+        L.vxo_filter_range.restype = U64
+        L.vxo_filter_range.argtypes = [ctypes.c_char_p, ctypes.c_int, ctypes.c_int, U64, U64, U64, U64,
+                                       _p64, _p64, U64]
+        L.vxo_table1_from_records.restype = ctypes.c_int
+        L.vxo_table1_from_records.argtypes = [ctypes.c_int, U64, U64, U64, _p64, _p64, _p64, _p64, _p64]
+        L.vxo_table2_digest.restype = U64
+        L.vxo_table2_digest.argtypes = [ctypes.c_int, ctypes.c_int, U64, U64, _p64, _p64, _p64, _p64, _p64]
         L.vxo_table1_digest.restype = ctypes.c_int
         L.vxo_table1_digest.argtypes = [ctypes.c_int, ctypes.c_char_p, ctypes.c_int, _p64, _p64]
         _lib = L
@@ -147,6 +154,89 @@ def table1_slice(K: int, key: bytes, bucket_bits: int, b_begin: int, b_end: int,
     if kept == UINT64_MAX:
         raise RuntimeError("vxo_table1_slice: capacity too small or out of memory")
     return offsets, nonces[:kept].copy(), hashes[:kept].copy()
+
+
+def filter_range(key: bytes, nsize: int, bucket_bits: int, b_begin: int, b_end: int, n_begin: int, n_end: int,
+                 cap: int):
+    """Records (nonces, hashes) of the nonces [n_begin, n_end) whose bucket lies in [b_begin, b_end)."""
+    nonces = np.empty(max(cap, 1), dtype=np.uint64)
+    hashes = np.empty(max(cap, 1), dtype=np.uint64)
+    kept = lib().vxo_filter_range(key, nsize, bucket_bits, b_begin, b_end, n_begin, n_end,
+                                  _ptr(nonces), _ptr(hashes), cap)
+    if kept == UINT64_MAX:
+        raise RuntimeError("vxo_filter_range: capacity too small")
+    return nonces[:kept].copy(), hashes[:kept].copy()
+
+
+def table1_from_records(bucket_bits: int, b_begin: int, b_end: int, nonces_in, hashes_in):
+    """Canonical Table 1 of the bucket range from its records in any order: (offsets, nonces, hashes)."""
+    nonces_in = np.ascontiguousarray(nonces_in, dtype=np.uint64)
+    hashes_in = np.ascontiguousarray(hashes_in, dtype=np.uint64)
+    cnt = len(nonces_in)
+    assert len(hashes_in) == cnt
+    offsets = np.empty(b_end - b_begin + 1, dtype=np.uint64)
+    nonces = np.empty(max(cnt, 1), dtype=np.uint64)
+    hashes = np.empty(max(cnt, 1), dtype=np.uint64)
+    rc = lib().vxo_table1_from_records(bucket_bits, b_begin, b_end, cnt, _ptr(nonces_in), _ptr(hashes_in),
+                                       _ptr(offsets), _ptr(nonces), _ptr(hashes))
+    if rc != 0:
+        raise RuntimeError(f"vxo_table1_from_records failed: {rc}")
+    return offsets, nonces[:cnt], hashes[:cnt]
+
+
+def table1_slice_parallel(K: int, key: bytes, bucket_bits: int, b_begin: int, b_end: int, workers: int):
+    """vxo_table1_slice with the hashing shared by `workers` threads, each running the single-threaded
+    vxo_filter_range on its own nonce range (ctypes releases the GIL for the call; the C code keeps no
+    global state).  Same result as table1_slice."""
+    from concurrent.futures import ThreadPoolExecutor
+    N = 1 << K
+    nsize = nonce_size(K)
+    pieces = max(workers * 4, 1)
+    bounds = [N * i // pieces for i in range(pieces + 1)]
+    expect = (N >> bucket_bits) * (b_end - b_begin) if K >= bucket_bits else (b_end - b_begin)
+    cap = max(1024, (2 * expect) // pieces + 8 * int((expect / pieces) ** 0.5) + 64)
+    lib()
+
+    def work(i):
+        return filter_range(key, nsize, bucket_bits, b_begin, b_end, bounds[i], bounds[i + 1], cap)
+
+    with ThreadPoolExecutor(max_workers=max(workers, 1)) as ex:
+        parts = list(ex.map(work, range(pieces)))
+    non = np.concatenate([p[0] for p in parts]) if parts else np.empty(0, dtype=np.uint64)
+    has = np.concatenate([p[1] for p in parts]) if parts else np.empty(0, dtype=np.uint64)
+    return table1_from_records(bucket_bits, b_begin, b_end, non, has)
+
+
+def hash_range_parallel(key: bytes, nsize: int, n_begin: int, count: int, workers: int) -> np.ndarray:
+    """hash_range with the range split over `workers` threads (each call is the single-threaded C loop)."""
+    from concurrent.futures import ThreadPoolExecutor
+    out = np.empty(count, dtype=np.uint64)
+    pieces = max(workers * 4, 1)
+    bounds = [count * i // pieces for i in range(pieces + 1)]
+    L = lib()
+
+    def work(i):
+        lo, hi = bounds[i], bounds[i + 1]
+        if hi > lo:
+            L.vxo_hash_range(key, nsize, n_begin + lo, hi - lo, _ptr(out[lo:hi]))
+
+    with ThreadPoolExecutor(max_workers=max(workers, 1)) as ex:
+        list(ex.map(work, range(pieces)))
+    return out
+
+
+def table2_digest(K: int, t1_offsets, nonces, hashes, mode: int = 1, b_begin: int = 0, b_end: int | None = None):
+    """(count2[nb], D2[nb]) of the bucket range of a canonical Table 1: D2[b] = sum f(f(n1) ^ n2) mod 2^64."""
+    if b_end is None:
+        b_end = len(t1_offsets) - 1
+    nb = b_end - b_begin
+    count2 = np.empty(max(nb, 1), dtype=np.uint64)
+    D2 = np.empty(max(nb, 1), dtype=np.uint64)
+    total = lib().vxo_table2_digest(K, mode, b_begin, b_end, _ptr(t1_offsets), _ptr(nonces), _ptr(hashes),
+                                    _ptr(count2), _ptr(D2))
+    if total == UINT64_MAX:
+        raise MemoryError
+    return count2[:nb], D2[:nb]
 
 
 def table1_digest(K: int, key: bytes, bucket_bits: int = 24):

@@ -25,7 +25,8 @@
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): the BLAKE3 routine against the independent
  * `blake3` Python package and against worked values in tests/golden/; SplitMix64 against its
  * published sequence; bucketing against invariants and the Poisson closed form; Step 4 against
- * Step 4' and against an independent numpy brute force and the closed form E|T2|.
+ * Step 4' and against an independent numpy brute force and the closed form E|T2|; the slice halves
+ * and the digest modes (large-K parity) against the full-table mode and plain-Python restatements.
  * Parity UNPINNED: agreement with the paper's own plot files / the VaultX prover (the paper prints
  * no table contents and VaultX is unpublished).
  */
@@ -364,40 +365,74 @@ static uint64_t mix64(uint64_t z)
 }
 uint64_t vxo_mix64(uint64_t z) { return mix64(z); }
 
-/* Slice mode for K too large to hold on the host: hashes ALL 2^K nonces but keeps only the
- * records whose bucket lies in [b_begin, b_end); returns them canonically (as vxo_table1 does for
- * the whole table) with offsets relative to b_begin.  cap = capacity of nonces/hashes.
- * Returns the number of records kept, or UINT64_MAX if cap is too small / out of memory. */
+/* Slice mode for K too large to hold on the host, in two halves so that several single-threaded
+ * workers can share the hashing (SURVEY.md 8(c) "Large-K parity": "run the slices as independent
+ * single-threaded processes on separate cores"):
+ *   vxo_filter_range        hashes the nonces [n_begin, n_end) and keeps, in nonce order, the records
+ *                           whose bucket lies in [b_begin, b_end)               (Steps 2 and 3)
+ *   vxo_table1_from_records puts records given in ANY order into the canonical form of vxo_table1 for
+ *                           that bucket range: offsets relative to b_begin, buckets sorted by (H, n)
+ * vxo_table1_slice is the one after the other over all 2^K nonces. */
+uint64_t vxo_filter_range(const uint8_t key[32], int nonce_size, int bucket_bits, uint64_t b_begin, uint64_t b_end,
+                          uint64_t n_begin, uint64_t n_end, uint64_t *nonces, uint64_t *hashes, uint64_t cap)
+{ /* returns the number of records kept, or UINT64_MAX if cap is too small */
+    uint64_t n, kept = 0;
+    for (n = n_begin; n < n_end; n++) {
+        const uint64_t H = vxo_hash_nonce(key, n, nonce_size);
+        const uint64_t b = H >> (64 - bucket_bits);
+        if (b < b_begin || b >= b_end) continue;
+        if (kept == cap) return UINT64_MAX;
+        nonces[kept] = n; hashes[kept] = H; kept++;
+    }
+    return kept;
+}
+
+int vxo_table1_from_records(int bucket_bits, uint64_t b_begin, uint64_t b_end, uint64_t cnt,
+                            const uint64_t *nonces_in, const uint64_t *hashes_in,
+                            uint64_t *offsets, uint64_t *nonces, uint64_t *hashes)
+{ /* 0, -1 a record outside the bucket range, -2 no memory */
+    const uint64_t nb = b_end - b_begin;
+    uint64_t i, b, *fill;
+    rec_t *rec;
+    rec = (rec_t *)malloc((size_t)(cnt ? cnt : 1) * sizeof *rec);
+    fill = (uint64_t *)calloc((size_t)(nb ? nb : 1), sizeof *fill);
+    if (!rec || !fill) { free(rec); free(fill); return -2; }
+    for (b = 0; b <= nb; b++) offsets[b] = 0;
+    for (i = 0; i < cnt; i++) {
+        b = hashes_in[i] >> (64 - bucket_bits);
+        if (b < b_begin || b >= b_end) { free(rec); free(fill); return -1; }
+        offsets[b - b_begin + 1]++;
+    }
+    for (b = 0; b < nb; b++) offsets[b + 1] += offsets[b];   /* exact-size buckets (A8) */
+    for (i = 0; i < cnt; i++) {
+        b = (hashes_in[i] >> (64 - bucket_bits)) - b_begin;
+        rec[offsets[b] + fill[b]].H = hashes_in[i];
+        rec[offsets[b] + fill[b]].n = nonces_in[i];
+        fill[b]++;
+    }
+    for (b = 0; b < nb; b++)                                  /* canonical in-bucket order (A10) */
+        if (offsets[b + 1] - offsets[b] > 1)
+            qsort(rec + offsets[b], (size_t)(offsets[b + 1] - offsets[b]), sizeof *rec, rec_cmp);
+    for (i = 0; i < cnt; i++) { nonces[i] = rec[i].n; hashes[i] = rec[i].H; }
+    free(rec); free(fill);
+    return 0;
+}
+
+/* hashes ALL 2^K nonces but keeps only the records whose bucket lies in [b_begin, b_end); returns
+ * them canonically (as vxo_table1 does for the whole table) with offsets relative to b_begin.
+ * cap = capacity of nonces/hashes.  Returns the number of records kept, or UINT64_MAX if cap is
+ * too small / out of memory. */
 uint64_t vxo_table1_slice(int K, const uint8_t key[32], int bucket_bits, uint64_t b_begin, uint64_t b_end,
                           uint64_t *offsets, uint64_t *nonces, uint64_t *hashes, uint64_t cap)
 {
-    const uint64_t N = 1ULL << K, nb = b_end - b_begin;
-    const int ns = vxo_nonce_size(K);
-    uint64_t n, b, kept = 0, *fill;
-    rec_t *rec, *raw;
-    raw = (rec_t *)malloc((size_t)(cap ? cap : 1) * sizeof *raw);
-    rec = (rec_t *)malloc((size_t)(cap ? cap : 1) * sizeof *rec);
-    fill = (uint64_t *)calloc((size_t)(nb ? nb : 1), sizeof *fill);
-    if (!raw || !rec || !fill) { free(raw); free(rec); free(fill); return UINT64_MAX; }
-    for (b = 0; b <= nb; b++) offsets[b] = 0;
-    for (n = 0; n < N; n++) {
-        const uint64_t H = vxo_hash_nonce(key, n, ns);
-        b = H >> (64 - bucket_bits);
-        if (b < b_begin || b >= b_end) continue;
-        if (kept == cap) { free(raw); free(rec); free(fill); return UINT64_MAX; }
-        raw[kept].H = H; raw[kept].n = n; kept++;
-        offsets[b - b_begin + 1]++;
-    }
-    for (b = 0; b < nb; b++) offsets[b + 1] += offsets[b];
-    for (n = 0; n < kept; n++) {
-        b = (raw[n].H >> (64 - bucket_bits)) - b_begin;
-        rec[offsets[b] + fill[b]++] = raw[n];
-    }
-    for (b = 0; b < nb; b++)
-        if (offsets[b + 1] - offsets[b] > 1)
-            qsort(rec + offsets[b], (size_t)(offsets[b + 1] - offsets[b]), sizeof *rec, rec_cmp);
-    for (n = 0; n < kept; n++) { nonces[n] = rec[n].n; hashes[n] = rec[n].H; }
-    free(raw); free(rec); free(fill);
+    uint64_t kept, *rn, *rh;
+    rn = (uint64_t *)malloc((size_t)(cap ? cap : 1) * sizeof *rn);
+    rh = (uint64_t *)malloc((size_t)(cap ? cap : 1) * sizeof *rh);
+    if (!rn || !rh) { free(rn); free(rh); return UINT64_MAX; }
+    kept = vxo_filter_range(key, vxo_nonce_size(K), bucket_bits, b_begin, b_end, 0, 1ULL << K, rn, rh, cap);
+    if (kept != UINT64_MAX && vxo_table1_from_records(bucket_bits, b_begin, b_end, kept, rn, rh, offsets, nonces, hashes) != 0)
+        kept = UINT64_MAX;
+    free(rn); free(rh);
     return kept;
 }
 
@@ -417,6 +452,37 @@ int vxo_table1_digest(int K, const uint8_t key[32], int bucket_bits, uint64_t *c
         D1[b] += mix64(H ^ mix64(n));
     }
     return 0;
+}
+
+/* Table-2 digest mode: count2[b] and D2[b] (above) for the buckets [b_begin, b_end) of a canonical
+ * Table 1, entries relative to b_begin.  Bucket by bucket it is Step 4 (mode 0) or Step 4' (mode 1)
+ * exactly as vxo_table2 runs them; only the records are folded into the digest instead of being kept.
+ * Returns the number of Table-2 records, UINT64_MAX if out of memory. */
+uint64_t vxo_table2_digest(int K, int mode, uint64_t b_begin, uint64_t b_end,
+                           const uint64_t *t1_offsets, const uint64_t *nonces, const uint64_t *hashes,
+                           uint64_t *count2, uint64_t *D2)
+{
+    uint64_t b, total = 0;
+    for (b = b_begin; b < b_end; b++) {
+        const uint64_t o = t1_offsets[b], c = t1_offsets[b + 1] - o;
+        uint64_t m, i, d = 0, *p1 = NULL, *p2 = NULL;
+        m = mode == 0 ? vxo_match_allpairs(K, c, nonces + o, hashes + o, NULL, NULL, 0)
+                      : vxo_match_sorted(K, c, nonces + o, hashes + o, NULL, NULL, 0);
+        if (m == UINT64_MAX) return UINT64_MAX;
+        if (m) {
+            p1 = (uint64_t *)malloc((size_t)m * sizeof *p1);
+            p2 = (uint64_t *)malloc((size_t)m * sizeof *p2);
+            if (!p1 || !p2) { free(p1); free(p2); return UINT64_MAX; }
+            if (mode == 0) vxo_match_allpairs(K, c, nonces + o, hashes + o, p1, p2, m);
+            else vxo_match_sorted(K, c, nonces + o, hashes + o, p1, p2, m);
+            for (i = 0; i < m; i++) d += mix64(mix64(p1[i]) ^ p2[i]);
+            free(p1); free(p2);
+        }
+        count2[b - b_begin] = m;
+        D2[b - b_begin] = d;
+        total += m;
+    }
+    return total;
 }
 
 /* ------------------------------------------------------------------ tiny CLI / timing ------- */

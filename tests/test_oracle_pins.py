@@ -291,6 +291,71 @@ def test_slice_and_digest_modes_agree_with_full_table():
         assert oracle.mix64(0) == 0 and oracle.mix64(1) == int(f(np.array([1], dtype=np.uint64))[0])
 
 
+def _py_mix64(z: int) -> int:
+    """SplitMix64 finaliser in plain Python integers (the digest function f of SURVEY.md 8(c))."""
+    M = (1 << 64) - 1
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & M
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & M
+    return z ^ (z >> 31)
+
+
+@pytest.mark.parametrize("K,B,seed,mode", [(10, 4, 3, 0), (12, 8, 1, 0), (12, 8, 1, 1), (16, 12, 1, 1), (14, 24, 5, 1)])
+def test_table2_digest_mode_agrees_with_full_table(K, B, seed, mode):
+    """count2[b] / D2[b] = sum f(f(n1) ^ n2) against the same quantities worked out in plain Python
+    from the full-table mode (itself pinned by brute force and the golden counts above)."""
+    key = vx_inputs.key_from_seed(seed)
+    off, non, has = oracle.table1(K, key, B)
+    t2o, n1, n2 = oracle.table2(K, off, non, has, mode)
+    c2, D2 = oracle.table2_digest(K, off, non, has, mode)
+    assert np.array_equal(c2, np.diff(t2o))
+    M = (1 << 64) - 1
+    want = [0] * (1 << B)
+    for b in np.flatnonzero(np.diff(t2o)):
+        acc = 0
+        for i in range(int(t2o[b]), int(t2o[b + 1])):
+            acc = (acc + _py_mix64(_py_mix64(int(n1[i])) ^ int(n2[i]))) & M
+        want[int(b)] = acc
+    assert [int(x) for x in D2] == want
+    # a bucket range gives the same entries
+    lo, hi = (1 << B) // 3, (1 << B) // 3 + min(50, (1 << B) // 2)
+    c2r, D2r = oracle.table2_digest(K, off, non, has, mode, lo, hi)
+    assert np.array_equal(c2r, c2[lo:hi]) and np.array_equal(D2r, D2[lo:hi])
+    # swapping the two nonces of a pair changes the digest (it is not symmetric in n1, n2)
+    assert _py_mix64(_py_mix64(5) ^ 9) != _py_mix64(_py_mix64(9) ^ 5)
+
+
+def test_slice_halves_and_parallel_helpers_agree_with_full_table():
+    """vxo_filter_range + vxo_table1_from_records (the two halves of the slice mode, used by the
+    large-K GPU tests with the hashing shared by several threads) against the full table."""
+    K, B = 15, 9
+    key = vx_inputs.key_from_seed(91)
+    off, non, has = oracle.table1(K, key, B)
+    b0, b1 = 100, 333
+    lo, hi = int(off[b0]), int(off[b1])
+    # records of a nonce range, in nonce order, with their library hashes
+    rn, rh = oracle.filter_range(key, 4, B, b0, b1, 1000, 20000, 1 << K)
+    H = lib_hashes(key, K)
+    sel = [n for n in range(1000, 20000) if b0 <= (int(H[n]) >> (64 - B)) < b1]
+    assert [int(x) for x in rn] == sel and [int(x) for x in rh] == [int(H[n]) for n in sel]
+    with pytest.raises(RuntimeError):
+        oracle.filter_range(key, 4, B, b0, b1, 0, 1 << K, 10)          # capacity too small
+    # any input order -> canonical form
+    an, ah = oracle.filter_range(key, 4, B, b0, b1, 0, 1 << K, 1 << K)
+    perm = np.random.default_rng(5).permutation(len(an))
+    so, sn, sh = oracle.table1_from_records(B, b0, b1, an[perm], ah[perm])
+    assert np.array_equal(so, off[b0:b1 + 1] - off[b0])
+    assert np.array_equal(sn, non[lo:hi]) and np.array_equal(sh, has[lo:hi])
+    with pytest.raises(RuntimeError):
+        oracle.table1_from_records(B, b0 + 1, b1, an, ah)              # a record outside the range
+    for workers in (1, 3):
+        po, pn, ph = oracle.table1_slice_parallel(K, key, B, b0, b1, workers)
+        assert np.array_equal(po, so) and np.array_equal(pn, sn) and np.array_equal(ph, sh)
+        assert np.array_equal(oracle.hash_range_parallel(key, 4, 77, 5000, workers), H[77:5077])
+    # the whole table through the halves
+    fo, fn, fh = oracle.table1_from_records(B, 0, 1 << B, np.arange(1 << K, dtype=np.uint64), H)
+    assert np.array_equal(fo, off) and np.array_equal(fn, non) and np.array_equal(fh, has)
+
+
 def test_K24_golden_histogram_and_match_count():
     # the plain oracle needs ~15 s here; this is the largest full-table pin (mean 1 record/bucket)
     (row,) = [r for r in _rows("bucket_histograms.txt") if r[0] == "24"]
