@@ -53,8 +53,10 @@ typedef enum {
     VX_ERR_CUDA = -4,      /* a CUDA runtime call failed; text in vx_last_error                    */
     VX_ERR_OVERFLOW = -5,  /* a partition's slack or the Table-2 capacity overflowed on the device */
     VX_ERR_RANGE = -6,     /* bucket range outside [0, 2^B] or records_capacity too small          */
-    VX_ERR_UNSUPPORTED = -7, /* a valid configuration this call does not implement                    */
-    VX_ERR_IO = -8          /* write() to the egress file descriptor failed; text in vx_last_error    */
+    VX_ERR_UNSUPPORTED = -7, /* a valid request beyond a fixed limit of this build (e.g. more than 16
+                                Table-2 egress calls in flight in one process); text in vx_last_error   */
+    VX_ERR_IO = -8,         /* write() to the egress file descriptor failed; text in vx_last_error    */
+    VX_ERR_NOMEM = -9       /* host memory for the handle could not be allocated                      */
 } vx_status;
 
 /* Device bytes the caller must provide for a plot of this K (B = 24 buckets bits, the paper's
@@ -169,10 +171,21 @@ vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64
  * synchronising call instead of dropping records silently (reading A8). */
 #define VX_OPT_PARTITION_CAPACITY_LIMIT 2
 #define VX_OPT_TABLE2_CAPACITY_LIMIT 3
+/* VX_OPT_SUBKEY_BITS (0 .. 32, default 32): how many hash bits below the bin index the fused kernel's
+ * fast in-bin ranking compares.  Fewer bits make records of one bin tie, come out in the wrong order
+ * and so send the tile through its "redo with exact (H, n) ranks" path (taken about once per 2^21
+ * tiles otherwise) -- results are identical by construction; tests use it to run that path. */
+#define VX_OPT_SUBKEY_BITS 4
 vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value);
 
 /* Synchronises; any output pointer may be NULL.  max_bucket = largest Table-1 bucket. */
 vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, uint32_t *max_bucket);
+
+/* Synchronises.  tile_retries = tiles of the last stage 2 whose fast in-bin ranking met a tie (two
+ * records of a bin with equal compared sub-keys, among them equal 64-bit hashes, reading A10) and
+ * which were therefore re-ranked by exact (H, n) compares; ~2^-21 per tile at the default 32
+ * sub-key bits.  For tests of that path (VX_OPT_SUBKEY_BITS). */
+vx_status vx_get_counters(vx_plot *p, uint64_t *tile_retries);
 
 /* Wait for the plot's enqueued work and report device-raised errors. */
 vx_status vx_synchronize(vx_plot *p);

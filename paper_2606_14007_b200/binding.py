@@ -17,17 +17,18 @@ VX_OK = 0
 VX_OPT_FORCE_EXACT_RANK = 1
 VX_OPT_PARTITION_CAPACITY_LIMIT = 2
 VX_OPT_TABLE2_CAPACITY_LIMIT = 3
+VX_OPT_SUBKEY_BITS = 4
 VX_CREATE_WIDE_LAYOUT = 1
 VX_CREATE_BIG_TILES = 2
 STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",
-          -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED", -8: "VX_ERR_IO"}
+          -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED", -8: "VX_ERR_IO", -9: "VX_ERR_NOMEM"}
 
 #: every symbol include/vx.h declares
 EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_opts", "vx_plot_create",
            "vx_plot_create_ex", "vx_plot_create_opts",
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
            "vx_sort_match_table2_to_file", "vx_read_tables",
-           "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_synchronize", "vx_hash_range",
+           "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
 
@@ -93,6 +94,8 @@ def load_library() -> ctypes.CDLL:
     L.vx_plot_set_option.argtypes = [_vp, ctypes.c_int, _u64]
     L.vx_get_stats.restype = ctypes.c_int
     L.vx_get_stats.argtypes = [_vp, ctypes.POINTER(_u64), ctypes.POINTER(_u64), ctypes.POINTER(_u32)]
+    L.vx_get_counters.restype = ctypes.c_int
+    L.vx_get_counters.argtypes = [_vp, ctypes.POINTER(_u64)]
     L.vx_synchronize.restype = ctypes.c_int
     L.vx_synchronize.argtypes = [_vp]
     L.vx_hash_range.restype = ctypes.c_int
@@ -119,10 +122,10 @@ def workspace_bytes(K: int, bucket_bits: int = 24, flags: int = 0) -> int:
     return int(load_library().vx_workspace_bytes_opts(K, bucket_bits, flags))
 
 
-def _stream_ptr(stream) -> int:
+def _stream_ptr(stream, device=None) -> int:
     import torch
     if stream is None:
-        stream = torch.cuda.current_stream()
+        stream = torch.cuda.current_stream(device)
     return int(stream.cuda_stream)
 
 
@@ -168,6 +171,14 @@ class Plot:
             self._check(self._L.vx_plot_bind(self._h, workspace.data_ptr(), workspace.numel()))
 
     # -- plumbing -------------------------------------------------------------------------------
+    def _dev(self):
+        """Every ABI call runs with the plot's device current (kernels launch on the current device)."""
+        import torch
+        return torch.cuda.device(self.device)
+
+    def _sp(self, stream) -> int:
+        return _stream_ptr(stream, self.device)
+
     def _check(self, st: int):
         if st != VX_OK:
             raise VxError(st, self._L.vx_last_error(self._h).decode())
@@ -192,37 +203,49 @@ class Plot:
 
     # -- the hot path ---------------------------------------------------------------------------
     def build_table1(self, stream=None):
-        self._check(self._L.vx_build_table1(self._h, _stream_ptr(stream)))
+        with self._dev():
+            self._check(self._L.vx_build_table1(self._h, self._sp(stream)))
 
     def sort_match_table2(self, stream=None):
-        self._check(self._L.vx_sort_match_table2(self._h, _stream_ptr(stream)))
+        with self._dev():
+            self._check(self._L.vx_sort_match_table2(self._h, self._sp(stream)))
 
     def sort_match_table2_to_host(self, copy_stream, records_ptr: int, records_capacity: int,
                                   offsets_ptr: int = 0, slices: int = 16, stream=None) -> int:
         """Stage 2 in `slices` launches with Table 2 streamed to host memory on copy_stream
         (vx_sort_match_table2_to_host); raw host pointers (pinned torch tensors); returns record bytes."""
         need = _sz()
-        self._check(self._L.vx_sort_match_table2_to_host(
-            self._h, _stream_ptr(stream), _stream_ptr(copy_stream), slices, records_ptr, records_capacity,
-            offsets_ptr or None, ctypes.byref(need)))
+        with self._dev():
+            self._check(self._L.vx_sort_match_table2_to_host(
+                self._h, self._sp(stream), self._sp(copy_stream), slices, records_ptr, records_capacity,
+                offsets_ptr or None, ctypes.byref(need)))
         return need.value
 
     def sort_match_table2_to_file(self, copy_stream, fd: int, staging_ptr: int, staging_bytes: int,
                                   slices: int = 16, stream=None) -> int:
         """Same, to a file descriptor through a pinned ring of 4 MB chunks; returns the bytes written."""
         n = _u64()
-        self._check(self._L.vx_sort_match_table2_to_file(
-            self._h, _stream_ptr(stream), _stream_ptr(copy_stream), slices, fd, staging_ptr, staging_bytes,
-            ctypes.byref(n)))
+        with self._dev():
+            self._check(self._L.vx_sort_match_table2_to_file(
+                self._h, self._sp(stream), self._sp(copy_stream), slices, fd, staging_ptr, staging_bytes,
+                ctypes.byref(n)))
         return n.value
 
     def synchronize(self):
-        self._check(self._L.vx_synchronize(self._h))
+        with self._dev():
+            self._check(self._L.vx_synchronize(self._h))
 
     def get_stats(self):
         t1, t2, mb = _u64(), _u64(), _u32()
-        self._check(self._L.vx_get_stats(self._h, ctypes.byref(t1), ctypes.byref(t2), ctypes.byref(mb)))
+        with self._dev():
+            self._check(self._L.vx_get_stats(self._h, ctypes.byref(t1), ctypes.byref(t2), ctypes.byref(mb)))
         return {"t1_records": t1.value, "t2_records": t2.value, "max_bucket": mb.value}
+
+    def get_counters(self):
+        r = _u64()
+        with self._dev():
+            self._check(self._L.vx_get_counters(self._h, ctypes.byref(r)))
+        return {"tile_retries": r.value}
 
     def read_tables(self, table: int, bucket_begin: int = 0, bucket_end: int | None = None,
                     records_out: np.ndarray | None = None):
@@ -232,22 +255,24 @@ class Plot:
         nb = bucket_end - bucket_begin
         offsets = np.empty(max(nb, 0) + 1, dtype=np.uint64)
         need = _sz()
-        self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
-                                           offsets.ctypes.data, None, 0, ctypes.byref(need)))
-        if records_out is None:
-            records_out = np.empty(need.value, dtype=np.uint8)
-        assert records_out.dtype == np.uint8 and records_out.flags.c_contiguous
-        self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
-                                           offsets.ctypes.data, records_out.ctypes.data,
-                                           records_out.nbytes, ctypes.byref(need)))
+        with self._dev():
+            self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
+                                               offsets.ctypes.data, None, 0, ctypes.byref(need)))
+            if records_out is None:
+                records_out = np.empty(need.value, dtype=np.uint8)
+            assert records_out.dtype == np.uint8 and records_out.flags.c_contiguous
+            self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
+                                               offsets.ctypes.data, records_out.ctypes.data,
+                                               records_out.nbytes, ctypes.byref(need)))
         return offsets, records_out[:need.value]
 
     def read_tables_into(self, table: int, bucket_begin: int, bucket_end: int,
                          offsets_ptr: int, records_ptr: int, records_capacity: int) -> int:
         """Raw-pointer form (e.g. pinned torch tensors): returns the record bytes written."""
         need = _sz()
-        self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
-                                           offsets_ptr, records_ptr, records_capacity, ctypes.byref(need)))
+        with self._dev():
+            self._check(self._L.vx_read_tables(self._h, table, bucket_begin, bucket_end,
+                                               offsets_ptr, records_ptr, records_capacity, ctypes.byref(need)))
         return need.value
 
     def set_option(self, option: int, value: int):
@@ -263,12 +288,13 @@ class Plot:
         """H(n) for n in [nonce_begin, nonce_begin+count) as a torch int64 CUDA tensor (bit pattern of u64)."""
         import torch
         out = torch.empty(count, dtype=torch.int64, device=self.device)
-        with torch.cuda.device(self.device):
-            self._check(self._L.vx_hash_range(self._h, nonce_begin, count, out.data_ptr(), _stream_ptr(stream)))
+        with self._dev():
+            self._check(self._L.vx_hash_range(self._h, nonce_begin, count, out.data_ptr(), self._sp(stream)))
         return out
 
     def hash_sink(self, count: int, sink, stream=None):
-        self._check(self._L.vx_hash_sink(self._h, count, sink.data_ptr(), sink.numel(), _stream_ptr(stream)))
+        with self._dev():
+            self._check(self._L.vx_hash_sink(self._h, count, sink.data_ptr(), sink.numel(), self._sp(stream)))
 
 
 def hash_range(K: int, key: bytes, nonce_begin: int, count: int):

@@ -21,8 +21,22 @@ def _nvcc() -> str:
     return exe
 
 
+STAMP = LIB + ".flags"      # the VX_NVCC_EXTRA string libvx.so was built with
+
+
+def _extra() -> str:
+    return " ".join(os.environ.get("VX_NVCC_EXTRA", "").split())      # e.g. -DVX_DEBUG_BOUNDS=1
+
+
 def is_stale() -> bool:
     if not os.path.exists(LIB):
+        return True
+    try:
+        with open(STAMP) as f:
+            built_with = f.read()
+    except OSError:
+        built_with = None
+    if built_with != _extra():     # a debug build must not stay behind as the product build, or vice versa
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS]
@@ -32,10 +46,12 @@ def is_stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/*.cu into paper_2606_14007_b200/libvx.so; returns its path."""
     if force or is_stale():
-        extra = os.environ.get("VX_NVCC_EXTRA", "").split()      # e.g. -DVX_S1_ITERS=4 (experiments)
+        extra = _extra().split()
         cmd = [_nvcc(), *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
                *[os.path.join(CSRC, s) for s in SOURCES]]
         subprocess.check_call(cmd, cwd=CSRC)
+        with open(STAMP, "w") as f:
+            f.write(_extra())
     return LIB
 
 

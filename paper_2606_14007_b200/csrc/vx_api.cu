@@ -6,6 +6,8 @@
 #include <string.h>
 #include <unistd.h>
 
+#include <atomic>
+#include <mutex>
 #include <new>
 
 #include "../../include/vx.h"
@@ -54,6 +56,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     // |T2| ~ 2^K (1 - 2^(B-K-1)) for K >= B, 2^(2K-1-B) below; sd ~ sqrt: 2^K + slack is ample
     g->t2_cap = g->N + (1u << 16);
     g->t2_check = g->t2_cap;
+    g->subkey_bits = 32;
     g->rec1_bytes = g->nonce_size + 8;
     g->rec2_bytes = 2 * g->nonce_size;
     size_t o = 0;
@@ -127,6 +130,17 @@ void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_s
 }
 
 // ------------------------------------------------------------------------------ helpers
+int vx_sm_count(void)
+{
+    static std::atomic<int> cache[64];
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (dev >= 0 && dev < 64 && (sms = cache[dev].load(std::memory_order_relaxed)) > 0) return sms;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return 148;
+    if (dev >= 0 && dev < 64) cache[dev].store(sms, std::memory_order_relaxed);
+    return sms;
+}
+
 static vx_status fail(vx_plot *p, vx_status s, const char *what)
 {
     if (p) snprintf(p->err, sizeof p->err, "%s: %s", vx_status_string(s), what);
@@ -172,6 +186,7 @@ const char *vx_status_string(vx_status s)
     case VX_ERR_RANGE: return "VX_ERR_RANGE";
     case VX_ERR_UNSUPPORTED: return "VX_ERR_UNSUPPORTED";
     case VX_ERR_IO: return "VX_ERR_IO";
+    case VX_ERR_NOMEM: return "VX_ERR_NOMEM";
     }
     return "VX_ERR_?";
 }
@@ -198,7 +213,7 @@ vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket
     VxGeom g;
     if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0, (flags & VX_CREATE_BIG_TILES) != 0)) return VX_ERR_ARG;
     vx_plot *p = new (std::nothrow) vx_plot;
-    if (!p) return VX_ERR_ARG;
+    if (!p) return VX_ERR_NOMEM;
     memset(p, 0, sizeof *p);
     p->g = g;
     memcpy(p->key, key, 32);
@@ -234,11 +249,15 @@ vx_status vx_plot_bind(vx_plot *p, void *dev_workspace, size_t bytes)
     if (e != cudaSuccess) return fail_cuda(p, e, "cudaDeviceGetAttribute");
     if (major < 10) return fail(p, VX_ERR_CUDA, "libvx is built for sm_100a only");
     p->num_sms = sms;
-    static uint64_t configured = 0;                        // one bit per device ordinal < 64
-    if (dev >= 64 || !(configured & (1ull << dev))) {
-        e = vx_stage2_configure();
-        if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute(stage 2 shared memory)");
-        if (dev < 64) configured |= 1ull << dev;
+    {
+        static std::mutex mu;                              // plots are bound from several host threads
+        static uint64_t configured = 0;                    // one bit per device ordinal < 64
+        std::lock_guard<std::mutex> lock(mu);
+        if (dev >= 64 || !(configured & (1ull << dev))) {
+            e = vx_stage2_configure();
+            if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute(stage 2 shared memory)");
+            if (dev < 64) configured |= 1ull << dev;
+        }
     }
     p->ws = (uint8_t *)dev_workspace;
     p->ws_bytes = bytes;
@@ -371,6 +390,7 @@ static vx_status egress_common(vx_plot *p, void *compute_stream, void *copy_stre
     if (soft == 1) return fail(p, VX_ERR_RANGE, msg);
     if (soft == 2) return fail(p, VX_ERR_OVERFLOW, msg);
     if (soft == 3) return fail(p, VX_ERR_IO, msg);
+    if (soft == 4) return fail(p, VX_ERR_UNSUPPORTED, msg);
     // both streams have drained inside vx_egress_run; the flags came back through the mailbox
     if (ctrl.flags & VX_FLAG_BOUNDS)
         return fail(p, VX_ERR_CUDA, "internal bounds check failed (VX_DEBUG_BOUNDS build)");
@@ -411,13 +431,8 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
         const uint32_t w[4] = {p->g.K, p->g.B, p->g.nonce_size, 0u};
         memcpy(tr + 8, w, 16);
         memcpy(tr + 24, &n, 8);
-        size_t left = sizeof tr;
-        const uint8_t *src = tr;
-        while (left) {
-            const ssize_t k = write(fd, src, left);
-            if (k < 0) return fail(p, VX_ERR_IO, "write(trailer) failed");
-            src += k; left -= (size_t)k; written += (uint64_t)k;
-        }
+        char msg[128];
+        if (vx_write_all(fd, tr, sizeof tr, &written, msg, sizeof msg)) s = fail(p, VX_ERR_IO, msg);
     }
     if (file_bytes) *file_bytes = written;
     return s;
@@ -450,6 +465,10 @@ vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value)
         if (value > p->g.t2_cap) return fail(p, VX_ERR_ARG, "limit above the Table-2 capacity");
         p->g.t2_check = value;
         return VX_OK;
+    case VX_OPT_SUBKEY_BITS:
+        if (value > 32) return fail(p, VX_ERR_ARG, "sub-key bits outside [0, 32]");
+        p->g.subkey_bits = (uint32_t)value;
+        return VX_OK;
     }
     return fail(p, VX_ERR_ARG, "unknown option");
 }
@@ -469,6 +488,19 @@ vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, u
     if (t1_records) *t1_records = t1;
     if (t2_records) *t2_records = p->state >= VX_MATCHED ? c.t2_total : 0;
     if (max_bucket) *max_bucket = p->t1_materialised ? c.max_bucket : 0;
+    return VX_OK;
+}
+
+vx_status vx_get_counters(vx_plot *p, uint64_t *tile_retries)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "vx_get_counters before vx_build_table1");
+    vx_status s = sync_and_check(p);
+    if (s != VX_OK) return s;
+    VxCtrl c;
+    cudaError_t e = cudaMemcpy(&c, p->ws + p->g.off_ctrl, sizeof c, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(ctrl)");
+    if (tile_retries) *tile_retries = c.retries;
     return VX_OK;
 }
 

@@ -49,8 +49,7 @@ static int mailbox_acquire(unsigned long long **host, unsigned long long **dev, 
             *dev = g_mb_dev + (size_t)i * VX_MAILBOX_WORDS;
             return i;
         }
-    *e = cudaErrorMemoryAllocation;                     // more than VX_MAILBOXES egress calls in flight
-    return -1;
+    return -1;                                          // *e == cudaSuccess: more than VX_MAILBOXES egress calls in flight
 }
 
 static void mailbox_release(int i)
@@ -74,22 +73,28 @@ struct VxRing {
     uint64_t written;
 };
 
+// write() until everything is out: EINTR is retried, a 0-byte write is an error (it would spin);
+// *written grows by the bytes that did go out.  Shared by the ring and the trailer (vx_api.cu).
+int vx_write_all(int fd, const uint8_t *src, size_t left, uint64_t *written, char *err, size_t errlen)
+{
+    while (left) {
+        const ssize_t w = write(fd, src, left);
+        if (w < 0 && errno == EINTR) continue;
+        if (w <= 0) {
+            snprintf(err, errlen, "write: %s", w < 0 ? strerror(errno) : "wrote 0 bytes");
+            return -1;
+        }
+        src += w; left -= (size_t)w; *written += (uint64_t)w;
+    }
+    return 0;
+}
+
 static int ring_write_oldest(VxRing *r, char *err, size_t errlen)
 {
     const size_t slot = r->tail % r->slots;
     cudaError_t e = cudaEventSynchronize(r->ev[slot]);
     if (e != cudaSuccess) { snprintf(err, errlen, "cudaEventSynchronize: %s", cudaGetErrorString(e)); return -1; }
-    const uint8_t *src = r->base + slot * VX_EGRESS_CHUNK;
-    size_t left = r->bytes[slot];
-    while (left) {
-        const ssize_t w = write(r->fd, src, left);
-        if (w < 0) {
-            if (errno == EINTR) continue;
-            snprintf(err, errlen, "write: %s", strerror(errno));
-            return -1;
-        }
-        src += w; left -= (size_t)w; r->written += (uint64_t)w;
-    }
+    if (vx_write_all(r->fd, r->base + slot * VX_EGRESS_CHUNK, r->bytes[slot], &r->written, err, errlen)) return -1;
     r->tail++;
     return 0;
 }
@@ -126,7 +131,13 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
     uint32_t made = 0;
     cudaError_t e;
     const int mailbox = mailbox_acquire(&ends, &ends_dev, &e);
-    if (mailbox < 0) return e;
+    if (mailbox < 0) {
+        if (e == cudaSuccess) {
+            *soft_error = 4;
+            snprintf(err, errlen, "more than %d Table-2 egress calls in flight in this process", VX_MAILBOXES);
+        }
+        return e;
+    }
     memset(ends, 0, slices * sizeof(unsigned long long));
     for (; e == cudaSuccess && made < slices; made++)
         e = cudaEventCreateWithFlags(&ev[made], cudaEventDisableTiming);

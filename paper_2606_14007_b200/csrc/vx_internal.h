@@ -34,6 +34,8 @@ struct VxGeom {
     uint32_t cap;  // partition capacity in records (mean + slack, multiple of 32)
     uint32_t cap_check;   // = cap; a test hook lowers it (the slot stride stays cap) to raise the overflow error
     uint64_t t2_check;    // = t2_cap; likewise for Table 2
+    uint32_t subkey_bits; // = 32: hash bits below the bin index that stage 2's fast ranking compares; a test hook
+                          // narrows it so that the tie -> exact re-rank path of a tile runs under test
     uint64_t N;    // 2^K
     uint64_t P;    // 2^pb
     uint64_t NB;   // 2^B
@@ -63,7 +65,7 @@ struct VxCtrl {
     uint32_t ticket;      // stage-2 tile dispenser
     uint32_t flags;       // bit 0: partition slack overflow, bit 1: Table-2 capacity overflow
     uint32_t max_bucket;  // largest Table-1 bucket seen by stage 2
-    uint32_t pad0;
+    uint32_t retries;     // tiles that stage 2 re-ranked exactly after its fast ranking met a tie
     unsigned long long t2_total;  // number of Table-2 records
     unsigned long long pad1;
 };
@@ -111,7 +113,10 @@ cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t
                                 uint64_t *dev_sink, size_t sink_words, cudaStream_t st);
 // Table-2 egress (vx_egress.cu): stage 2 in `slices` partition-range launches on `compute`, each
 // finished slice copied on `copy` to host memory (host_records / host_offsets) or, through a pinned
-// ring of 4 MB chunks, to a file.  *soft_error: 0 ok, 1 capacity too small, 2 Table-2 overflow, 3 I/O.
+// ring of 4 MB chunks, to a file.  *soft_error: 0 ok, 1 capacity too small, 2 Table-2 overflow, 3 I/O,
+// 4 too many egress calls in flight.
+int vx_write_all(int fd, const uint8_t *src, size_t bytes, uint64_t *written, char *err, size_t errlen);
+int vx_sm_count(void);   // SMs of the current device (cached per ordinal); 148 if the query fails
 struct VxRing;
 VxRing *vx_ring_create(void *pinned, size_t bytes, int fd);   // NULL: fewer than two 4 MB chunks, or no memory
 uint64_t vx_ring_written(const VxRing *r);

@@ -131,7 +131,8 @@ cudaError_t vx_launch_clear(cudaStream_t st, void *a, size_t bytes_a, void *b, s
     const size_t na = (bytes_a + 15) / 16, nb = (bytes_b + 15) / 16;
     size_t grid = ((na > nb ? na : nb) + 255) / 256;
     if (grid < 1) grid = 1;
-    if (grid > 148 * 8) grid = 148 * 8;
+    const size_t gmax = (size_t)vx_sm_count() * 8;
+    if (grid > gmax) grid = gmax;
     vx_k_clear<<<(unsigned)grid, 256, 0, st>>>((uint4 *)a, na, (uint4 *)b, nb, w0, w1);
     return cudaGetLastError();
 }

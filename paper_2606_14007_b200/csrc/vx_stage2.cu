@@ -46,6 +46,7 @@ struct VxS2Params {
     unsigned long long *t2_off;
     unsigned long long N, NB, t2_cap;
     uint32_t P, cap, pb, fb, K, B, do_match, force_exact;
+    uint32_t submask;            // sub-key bits the fast ranking pass compares (~0; a test hook narrows it)
     // this launch sorts the partitions [tile_begin, tile_end): the whole plot, or one slice of it
     // when Table 2 is streamed to the host while later slices are still being matched (vx_egress.cu)
     uint32_t tile_begin, tile_end;
@@ -183,6 +184,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
     const int tid = threadIdx.x, lane = tid & 31, wbase = tid & ~31;
     const int sh = q.binshift - 32;                     // bin / sub-key shifts act on the high key word
+    const uint32_t submask = q.submask;
     const int bshift = q.bshift;
     const uint32_t fbmask = (1u << q.fb) - 1u;
     const uint64_t Tm1 = q.Tm1;                         // T - 1 in key units
@@ -326,7 +328,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         VX_CHECK(q.ctrl, pos < cnt);
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
-                        sub[pos] = vx_subkey(key[it], sh);
+                        sub[pos] = vx_subkey(key[it], sh) & submask;
                     }
                 }
             }
@@ -348,20 +350,23 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t nm = __reduce_max_sync(VX_FULL, n);
                     uint32_t rank = 0;
                     if (!exact) {
-                        // by the 32 bits below the bin index; equal sub-keys (or equal hashes) give
-                        // equal ranks, which phase E sees as keys that do not strictly increase
+                        // by (the 32 bits below the bin index, position in the bin): every record of a
+                        // bin gets a rank of its own, so no two lanes ever write one slot.  Records
+                        // with equal sub-keys (or equal hashes) may come out in the wrong order, which
+                        // phase E sees as keys that do not strictly increase
                         const uint32_t *sp = sub + s;
-                        const uint32_t ks = vx_subkey(k, sh);
+                        const uint32_t ks = vx_subkey(k, sh) & submask;
+                        const uint32_t me = i - s;
 #pragma unroll
                         for (uint32_t j = 0; j < 4; j++) {
                             const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
-                            rank += kj < ks ? 1u : 0u;
+                            rank += (kj < ks || (kj == ks && j < me)) ? 1u : 0u;
                         }
                         if (nm > 4) {
 #pragma unroll 1
                             for (uint32_t j = 4; j < nm; j++) {
                                 const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
-                                rank += kj < ks ? 1u : 0u;
+                                rank += (kj < ks || (kj == ks && j < me)) ? 1u : 0u;
                             }
                         }
                     } else {                            // by (H, n), reading A10
@@ -437,7 +442,11 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 }
             }
             __syncthreads();
-            if (!exact && s_tie) { exact = 1u; continue; }   // block-uniform: redo this tile exactly
+            if (!exact && s_tie) {                      // block-uniform: redo this tile exactly
+                if (tid == 0) atomicAdd(&q.ctrl->retries, 1u);
+                exact = 1u;
+                continue;
+            }
             break;
         }
         if (finished) break;
@@ -575,7 +584,7 @@ cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, ui
 {
     if (count == 0) return cudaSuccess;
     uint64_t grid = (count + 255) / 256;
-    if (grid > 148 * 16) grid = 148 * 16;
+    if (grid > (uint64_t)vx_sm_count() * 16) grid = (uint64_t)vx_sm_count() * 16;
     const uint4 *part = (const uint4 *)(ws + g.off_part);
     const uint16_t *part_b = (const uint16_t *)(ws + g.off_part_b);
     const unsigned long long *pbase = (const unsigned long long *)(ws + g.off_part_base);
@@ -594,7 +603,7 @@ cudaError_t vx_launch_export_t2(const VxGeom &g, uint8_t *ws, uint64_t first, ui
 {
     if (count == 0) return cudaSuccess;
     uint64_t grid = (count + 255) / 256;
-    if (grid > 148 * 16) grid = 148 * 16;
+    if (grid > (uint64_t)vx_sm_count() * 16) grid = (uint64_t)vx_sm_count() * 16;
     vx_k_export_t2<<<(unsigned)grid, 256, 0, st>>>((const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi,
                                                    first, count, ws + g.off_stage + stage_offset);
     return cudaGetLastError();
@@ -650,6 +659,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.cap_check = g.cap_check; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
+    q.submask = g.subkey_bits >= 32 ? ~0u : g.subkey_bits == 0 ? 0u : ~0u << (32 - g.subkey_bits);
     q.tile_begin = tile_begin; q.tile_end = tile_end; q.slice_end_out = slice_end_out;
     if (g.pb + g.tile_log > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
     q.part_b = (uint16_t *)(ws + g.off_part_b);

@@ -20,7 +20,12 @@ import pytest
 
 import oracle
 import vx_inputs
-from vx_testlib import canon_t2, decode_t1, decode_t2
+import os
+
+from vx_testlib import (canon_t2, decode_t1, decode_t2, t_lsr, torch_match_digest_chunk,
+                        torch_table2_digest)
+
+WORKERS = max(1, min(os.cpu_count() or 1, 64))     # threads sharing the oracle's hashing (each single-threaded C)
 
 pytestmark = pytest.mark.gpu
 
@@ -83,6 +88,10 @@ def device_views(plot):
     return part, pb, o1, o2, t2 - base
 
 
+def plot_key(plot):
+    return plot._test_key
+
+
 def whole_table_properties(plot, K):
     """Any-size properties over the whole of Table 1 and Table 2, on the device (torch)."""
     import torch
@@ -96,6 +105,11 @@ def whole_table_properties(plot, K):
     cnt = pb[1:] - pb[:-1]
     assert int(pb[0]) == 0 and int(pb[-1]) == N and int(cnt.max()) <= cap
     hashes = plot.hash_range(0, N)                       # int64 bit patterns of u64, indexed by nonce
+    # the stream itself against the oracle, hash by hash, on 2^17 nonces drawn over the whole range
+    pick = np.unique(np.random.default_rng(K).integers(0, N, 1 << 17))
+    got = hashes[torch.from_numpy(pick).to(dev)].cpu().numpy().view(np.uint64)
+    want = np.array([oracle.hash_nonce(plot_key(plot), int(n), 4) for n in pick], dtype=np.uint64)
+    assert np.array_equal(got, want), "the hash stream differs from the oracle"
     seen = torch.zeros(N, dtype=torch.bool, device=dev)
     lane = torch.arange(cap, device=dev)[None, :]
     chunk = max(1, min(P, (1 << 26) // cap))
@@ -126,8 +140,7 @@ def whole_table_properties(plot, K):
     # Table 2
     M = stats["t2_records"]
     assert int(o2[0]) == 0 and int(o2[-1]) == M and bool((o2[1:] >= o2[:-1]).all())
-    mean = N * (1 - 2.0 ** (B - K - 1)) if K >= B else 2.0 ** (2 * K - 1 - B)
-    assert abs(M - mean) < 6 * mean ** 0.5 + 8, (M, mean)
+    # (completeness of Table 2 is checked exactly, bucket by bucket, by whole_table2_digest_check)
     t2 = plot.workspace[t2_off_bytes: t2_off_bytes + M * 8].view(torch.int32).view(M, 2)
     T = 1 << (64 - K)
     step = 1 << 26
@@ -148,29 +161,145 @@ def whole_table_properties(plot, K):
     return stats
 
 
+def sorted_runs(plot, chunk_records=1 << 24):
+    """Table 1 as the kernels left it, in runs of whole partitions: yields (H, n) as int64 tensors,
+    H ascending (unsigned) within the run.  Narrow layout: 16-byte records; wide layout: the hash is
+    rebuilt from the partition index and a = (H << pb) | (n >> t), the nonce from a and b (include/vx.h)."""
+    import torch
+    pbits, cap, t = plot.partition_bits, plot.partition_capacity, plot.tile_log
+    P = 1 << pbits
+    dev = plot.device
+    lane = torch.arange(cap, device=dev)[None, :]
+    step = max(1, chunk_records // cap)
+    if plot.wide:
+        a, b, pb, o1, o2 = wide_views(plot)
+    else:
+        part, pb, o1, o2, _ = device_views(plot)
+    cnt = pb[1:] - pb[:-1]
+    for p0 in range(0, P, step):
+        p1 = min(P, p0 + step)
+        valid = lane < cnt[p0:p1, None]
+        if plot.wide:
+            ak = a[p0:p1][valid]
+            bk = (b[p0:p1].long() & 0xffff)[valid]
+            pid = torch.arange(p0, p1, device=dev)[:, None].expand(p1 - p0, cap)[valid]
+            H = t_lsr(ak, pbits) if pbits else ak
+            if pbits:
+                H = H | (pid << (64 - pbits))
+            n = ((ak & ((1 << pbits) - 1)) << t) | bk
+        else:
+            blk = part[p0:p1]
+            H = (((blk[..., 1].long() & 0xffffffff) << 32) | (blk[..., 0].long() & 0xffffffff))[valid]
+            n = (blk[..., 2].long() & 0xffffffff)[valid]
+        yield H, n
+
+
+def table2_records(plot, r0, r1):
+    """Table-2 records [r0, r1) of the device-resident table as (n1, n2) int64 tensors."""
+    import torch
+    t1, t1o, t2, t2o, pbase = plot.device_tables()
+    ws, base = plot.workspace, plot.workspace.data_ptr()
+    o = t2 - base
+    rec = ws[o + 8 * r0: o + 8 * r1].view(torch.int32).view(-1, 2)
+    n1 = rec[:, 0].long() & 0xffffffff
+    n2 = rec[:, 1].long() & 0xffffffff
+    if plot.nonce_size > 4:                              # packed: uint2 {n1 lo, n2 lo} + a byte of high bits
+        ho = (o + 8 * plot.t2_capacity + 255) & ~255
+        hi = ws[ho + r0: ho + r1].long()
+        n1 = n1 | ((hi & 15) << 32)
+        n2 = n2 | ((hi >> 4) << 32)
+    return n1, n2
+
+
+def whole_table2_digest_check(plot, K):
+    """EVERY bucket of Table 2 (count and content digest) against the torch restatement of the match
+    step applied to the sorted Table 1 on the device: no pair missing, none extra, none altered.
+    Returns (count2, D2) as uint64 numpy arrays (for the oracle comparison at K = 27)."""
+    import torch
+    B = plot.bucket_bits
+    NB = 1 << B
+    dev = plot.device
+    stats = plot.get_stats()
+    M = stats["t2_records"]
+    want_c = torch.zeros(NB, dtype=torch.int64, device=dev)
+    want_D = torch.zeros(NB, dtype=torch.int64, device=dev)
+    total = 0
+    for H, n in sorted_runs(plot):
+        total += torch_match_digest_chunk(H, n, K, B, want_c, want_D)
+        del H, n
+    assert total == M, (total, M)
+    t1, t1o, t2, t2o, pbase = plot.device_tables()
+    base = plot.workspace.data_ptr()
+    o2 = plot.workspace[t2o - base: t2o - base + (NB + 1) * 8].view(torch.int64)
+    assert bool((o2[1:] - o2[:-1] == want_c).all()), "a bucket's Table-2 count differs from the exact match count"
+    got_c = torch.zeros(NB, dtype=torch.int64, device=dev)
+    got_D = torch.zeros(NB, dtype=torch.int64, device=dev)
+    step = 1 << 25
+    for r0 in range(0, M, step):
+        r1 = min(M, r0 + step)
+        n1, n2 = table2_records(plot, r0, r1)
+        torch_table2_digest(n1, n2, o2, r0, got_c, got_D)
+        del n1, n2
+    assert bool((got_c == want_c).all())
+    assert bool((got_D == want_D).all()), "a bucket's Table-2 content digest differs from the exact match set"
+    return want_c.cpu().numpy().view(np.uint64), want_D.cpu().numpy().view(np.uint64)
+
+
+def check_oracle_slice(plot, K, key, b0, b1):
+    """Buckets [b0, b1): the oracle hashes ALL 2^K nonces (WORKERS threads, each the single-threaded
+    C loop on its own nonce range) and keeps this slice; Tables 1 and 2 of the slice byte for byte."""
+    B = plot.bucket_bits
+    so, sn, sh = oracle.table1_slice_parallel(K, key, B, b0, b1, WORKERS)
+    off1, raw1 = plot.read_tables(1, b0, b1)
+    assert np.array_equal(off1, so)
+    assert np.array_equal(raw1, oracle.serialize_t1(plot.nonce_size, sn, sh))
+    t2o, n1, n2 = oracle.table2(K, so, sn, sh, 1)
+    off2, raw2 = plot.read_tables(2, b0, b1)
+    assert np.array_equal(off2, t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, plot.nonce_size))
+    assert np.array_equal(g1, n1) and np.array_equal(g2, n2)
+    return len(sn)
+
+
 def test_digest_function_matches_the_oracles():
     z = np.array([0, 1, 0x0123456789abcdef, MASK64], dtype=np.uint64)
     assert [int(x) for x in np_mix64(z)] == [oracle.mix64(int(x)) for x in z]
 
 
-def test_K27_full_size_digests_and_samples(vx):
+def test_K27_full_size_every_bucket_vs_oracle(vx):
+    """BASELINE.json configs[1] in full: the oracle makes the whole plot (its hashing shared by WORKERS
+    threads); Table 1 is compared byte for byte, Table 2 bucket by bucket (count + content digest, all
+    2^24 buckets, SURVEY 8(c) "Large-K parity" (iii)), and the torch restatement of the match step that
+    the larger sizes rely on is compared with the oracle's digest as well."""
     K, B = 27, 24
+    N, NB = 1 << K, 1 << B
     key = vx_inputs.config_key(K)
     plot = vx.Plot(K, key, B)
+    plot._test_key = key
     plot.build_table1()
     plot.sort_match_table2()
-    count1, D1 = oracle.table1_digest(K, key, B)          # the oracle hashes all 2^27 nonces
+    H = oracle.hash_range_parallel(key, 4, 0, N, WORKERS)
+    off, non, has = oracle.table1_from_records(B, 0, NB, np.arange(N, dtype=np.uint64), H)
+    del H
     off1, raw1 = plot.read_tables(1)
-    assert np.array_equal(np.diff(off1), count1)
-    non, has = decode_t1(raw1, 4)
+    assert np.array_equal(off1, off)
+    assert np.array_equal(raw1, oracle.serialize_t1(4, non, has)), "Table 1 differs from the oracle's"
     del raw1
-    term = np_mix64(has ^ np_mix64(non))
+    count2, D2 = oracle.table2_digest(K, off, non, has, 1)
+    del non, has
+    off2, raw2 = plot.read_tables(2)
+    assert np.array_equal(np.diff(off2), count2), "a bucket's Table-2 size differs from the oracle's"
+    n1, n2 = decode_t2(raw2, 4)
+    del raw2
+    term = np_mix64(np_mix64(n1) ^ n2)
     cs = np.concatenate(([np.uint64(0)], np.cumsum(term, dtype=np.uint64)))
-    got = cs[off1[1:].astype(np.int64)] - cs[off1[:-1].astype(np.int64)]
-    assert np.array_equal(got, D1), "a bucket's content digest differs from the oracle's"
-    del term, cs, got, non, has
-    n = check_sampled_buckets(plot, K, key, [(0, 64), (12345, 12400), (8388600, 8388700), ((1 << 24) - 50, 1 << 24)])
-    assert n > 1500
+    got = cs[off2[1:].astype(np.int64)] - cs[off2[:-1].astype(np.int64)]
+    assert np.array_equal(got, D2), "a bucket's Table-2 content digest differs from the oracle's"
+    del term, cs, got, n1, n2
+    tc, tD = whole_table2_digest_check(plot, K)           # GPU Table 2 == torch matcher, every bucket ...
+    assert np.array_equal(tc, count2) and np.array_equal(tD, D2)   # ... and torch matcher == oracle
+    n = check_sampled_buckets(plot, K, key, [(0, 64), (8388600, 8388700), ((1 << 24) - 50, 1 << 24)])
+    assert n > 1000
     whole_table_properties(plot, K)
     plot.free()
 
@@ -188,15 +317,20 @@ def test_K29_K32_full_size_samples_and_properties(vx, K):
         pytest.skip(f"needs {need / 1e9:.0f} GB of device memory, {free / 1e9:.0f} GB free")
     key = vx_inputs.config_key(K)
     plot = vx.Plot(K, key, B)
-    assert plot.tile_log == (13 if K >= 32 else 12)
+    plot._test_key = key
     plot.build_table1()
     plot.sort_match_table2()
     rng = np.random.default_rng(K)
     starts = [0, (1 << 24) - 8] + [int(x) for x in rng.integers(0, (1 << 24) - 8, 14)]
     n = check_sampled_buckets(plot, K, key, [(s, s + 8) for s in starts])
     assert n > 3000
+    if K == 29:
+        # 2^13 consecutive buckets (two whole stage-2 tiles and their neighbours' edges) from the oracle,
+        # which hashes all 2^29 nonces for them
+        assert check_oracle_slice(plot, K, key, 5000 * 128 - 64, 5000 * 128 - 64 + (1 << 13)) > 250000
     stats = whole_table_properties(plot, K)
     assert stats["t1_records"] == 1 << K
+    whole_table2_digest_check(plot, K)
     plot.free()
 
 
@@ -204,6 +338,7 @@ def test_K31_full_size_samples_and_properties(vx):
     K, B = 31, 24
     key = vx_inputs.config_key(K)
     plot = vx.Plot(K, key, B)
+    plot._test_key = key
     plot.build_table1()
     plot.sort_match_table2()
     rng = np.random.default_rng(31)
@@ -212,6 +347,21 @@ def test_K31_full_size_samples_and_properties(vx):
     assert n > 20000
     stats = whole_table_properties(plot, K)
     assert stats["t1_records"] == 1 << 31
+    whole_table2_digest_check(plot, K)
+    plot.free()
+
+
+def test_K31_oracle_slice_of_4096_consecutive_buckets(vx):
+    """BASELINE.json configs[3]: 2^12 consecutive buckets (128 whole stage-2 tiles, ~2^19 records)
+    straight from the oracle, which hashes all 2^31 nonces for them (WORKERS threads); Tables 1 and 2
+    of the slice byte for byte.  The slice starts mid-tile so that tile edges are inside it."""
+    K, B = 31, 24
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    plot.sort_match_table2()
+    b0 = 11 * (1 << 20) + 13
+    assert check_oracle_slice(plot, K, key, b0, b0 + (1 << 12)) > 500000
     plot.free()
 
 

@@ -59,10 +59,12 @@ def test_hash_worked_values(vx):
 
 
 # ------------------------------------------------------------------ full tables, small K
-def run_plot(vx, K, key, B, force_exact=False, flags=0):
+def run_plot(vx, K, key, B, force_exact=False, flags=0, subkey_bits=None, counters=None):
     plot = vx.Plot(K, key, B, flags=flags)
     if force_exact:
         plot.set_option(vx.VX_OPT_FORCE_EXACT_RANK, 1)
+    if subkey_bits is not None:
+        plot.set_option(vx.VX_OPT_SUBKEY_BITS, subkey_bits)
     plot.build_table1()
     # Table 1 straight after stage 1: bucket order unspecified (A9) -> canonicalise
     off_b, raw_b = plot.read_tables(1)
@@ -70,6 +72,8 @@ def run_plot(vx, K, key, B, force_exact=False, flags=0):
     off1, raw1 = plot.read_tables(1)
     off2, raw2 = plot.read_tables(2)
     stats = plot.get_stats()
+    if counters is not None:
+        counters.update(plot.get_counters())
     nsize = plot.nonce_size
     plot.free()
     return (off_b, raw_b), (off1, raw1), (off2, raw2), stats, nsize
@@ -123,6 +127,45 @@ def test_exact_rerank_path_gives_the_same_tables(vx, K, B, seed):
     assert np.array_equal(off2, o_t2o)
     g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
     assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+
+
+# The fast ranking pass of the fused kernel compares 32 hash bits below the bin index; two records of
+# one bin that tie on them (about once per 2^21 tiles) may come out in the wrong order, which the
+# kernel sees as keys that do not strictly increase, and the tile is then redone with exact (H, n)
+# ranks -- with the deferred emit of the CTA's previous tile already spent.  VX_OPT_SUBKEY_BITS narrows
+# the compared bits so that this redo runs on most tiles; the tables must still be the oracle's.
+RETRY_LAYOUTS = [("narrow", 0), ("wide", 1), ("big", 2), ("big+wide", 3)]
+
+
+@pytest.mark.parametrize("bits", [0, 3])
+@pytest.mark.parametrize("layout,flags", RETRY_LAYOUTS)
+@pytest.mark.parametrize("K,B,seed", [(12, 8, 1), (13, 8, 4), (16, 12, 1), (16, 7, 6), (18, 12, 9), (18, 24, 3),
+                                      (20, 24, 1), (21, 12, 2), (22, 24, 22)])
+def test_tie_retry_path_gives_the_same_tables(vx, K, B, seed, layout, flags, bits):
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    ctr = {}
+    _, (off1, raw1), (off2, raw2), stats, nsize = run_plot(vx, K, key, B, flags=flags, subkey_bits=bits, counters=ctr)
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(nsize, o_non, o_has))
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(raw2, nsize))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    assert stats["t2_records"] == len(o_n1)
+    # dense tiles (several records per bin somewhere in nearly every tile): the redo did run
+    tile_log = 13 if flags & 2 else 12
+    tiles = 1 << max(K - tile_log, 0)
+    if K >= tile_log:
+        assert ctr["tile_retries"] >= tiles // 2, ctr
+    assert ctr["tile_retries"] <= tiles
+
+
+def test_default_subkey_bits_take_no_retry(vx):
+    K, B = 20, 24
+    key = vx_inputs.key_from_seed(1)
+    ctr = {}
+    run_plot(vx, K, key, B, counters=ctr)
+    assert ctr["tile_retries"] == 0
 
 
 WIDE_CASES = [(4, 2, 3), (10, 6, 2), (12, 8, 1), (12, 12, 7), (13, 8, 4), (16, 12, 1), (16, 7, 6),
