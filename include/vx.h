@@ -200,6 +200,20 @@ vx_status vx_hash_range(vx_plot *p, uint64_t nonce_begin, uint64_t count, uint64
 vx_status vx_hash_sink(vx_plot *p, uint64_t count, uint64_t *dev_sink, size_t sink_words,
                        void *cuda_stream);
 
+/* Measurement aid for the same roofline (the integer pipes' issue rate is not in
+ * MEASURED_PEAKS.json and is to be measured with dependent-free instruction chains): launches
+ * vx_sm_count x ctas_per_sm CTAs of 256 threads, each thread running 8 independent chains of
+ * 8 * iters instructions of one kind; *lane_ops = thread-instructions of that kind executed.
+ * dev_out: DEVICE scratch of >= 1024 uint32.  Enqueues only; the caller times it with CUDA events. */
+#define VX_PROBE_LOP3 0 /* a = a ^ b ^ c            (ALU pipe)                 */
+#define VX_PROBE_SHF 1  /* rotate                   (ALU pipe)                 */
+#define VX_PROBE_ADD 2  /* 32-bit add               (ptxas: IADD3 or IMAD.IADD) */
+#define VX_PROBE_IMAD 3 /* a = a * b + c            (FMA pipe)                 */
+#define VX_PROBE_PRMT 4 /* byte permute             (ALU pipe)                 */
+#define VX_PROBE_ARX 5  /* xor, rotate alternating  (BLAKE3's mix)             */
+vx_status vx_probe_alu(int kind, uint32_t iters, uint32_t ctas_per_sm, uint32_t *dev_out, size_t out_words,
+                       void *cuda_stream, uint64_t *lane_ops);
+
 /* Plot geometry, for tests and the bench report.  Any pointer may be NULL. */
 vx_status vx_plot_info(const vx_plot *p, uint32_t *K, uint32_t *bucket_bits, uint32_t *nonce_size,
                        uint32_t *partition_bits, uint32_t *partition_capacity, uint64_t *t2_capacity);

@@ -29,7 +29,7 @@ EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_op
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
            "vx_sort_match_table2_to_file", "vx_read_tables",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
-           "vx_hash_sink",
+           "vx_hash_sink", "vx_probe_alu",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
 
 _u64 = ctypes.c_uint64
@@ -102,6 +102,8 @@ def load_library() -> ctypes.CDLL:
     L.vx_hash_range.argtypes = [_vp, _u64, _u64, _vp, _vp]
     L.vx_hash_sink.restype = ctypes.c_int
     L.vx_hash_sink.argtypes = [_vp, _u64, _vp, _sz, _vp]
+    L.vx_probe_alu.restype = ctypes.c_int
+    L.vx_probe_alu.argtypes = [ctypes.c_int, _u32, _u32, _vp, _sz, _vp, ctypes.POINTER(_u64)]
     L.vx_plot_info.restype = ctypes.c_int
     L.vx_plot_info.argtypes = [_vp] + [ctypes.POINTER(_u32)] * 5 + [ctypes.POINTER(_u64)]
     L.vx_plot_layout.restype = ctypes.c_int
@@ -295,6 +297,19 @@ class Plot:
     def hash_sink(self, count: int, sink, stream=None):
         with self._dev():
             self._check(self._L.vx_hash_sink(self._h, count, sink.data_ptr(), sink.numel(), self._sp(stream)))
+
+
+PROBE_KINDS = {"lop3": 0, "shf": 1, "add": 2, "imad": 3, "prmt": 4, "arx": 5}
+
+
+def probe_alu(kind: str, iters: int, scratch, ctas_per_sm: int = 8, stream=None) -> int:
+    """vx_probe_alu: enqueue one dependent-free chain kernel; returns the lane-ops it executes."""
+    ops = _u64()
+    st = load_library().vx_probe_alu(PROBE_KINDS[kind], iters, ctas_per_sm, scratch.data_ptr(), scratch.numel(),
+                                     _stream_ptr(stream, scratch.device), ctypes.byref(ops))
+    if st != VX_OK:
+        raise VxError(st, f"vx_probe_alu({kind})")
+    return ops.value
 
 
 def hash_range(K: int, key: bytes, nonce_begin: int, count: int):

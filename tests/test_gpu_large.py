@@ -1,8 +1,7 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
 
-K = 27 (configs[1]): every bucket's count and order-independent digest against the oracle's
-streaming digest mode (the oracle hashes all 2^27 nonces), Table 2 of sampled bucket ranges
-bit-exact against the oracle, sortedness and completeness of the whole table.
+K = 27 (configs[1]): the oracle makes the whole plot; Table 1 byte for byte, Table 2 bucket by bucket
+(count + order-independent content digest, all 2^24 buckets), sortedness and completeness.
 
 K = 31 (configs[3], the configuration the metric is quoted on): the oracle cannot hash 2^31 nonces
 in test time, so
@@ -12,7 +11,10 @@ in test time, so
     every nonce exactly once, every partition sorted and inside its hash prefix, every record's H
     equal to the hash stream of vx_hash_range (itself compared with the oracle on sampled ranges in
     test_gpu_parity.py), every Table-2 entry inside one bucket with 0 <= H2 - H1 < T and
-    (H1, n1) < (H2, n2), CSR offsets consistent, |T2| within 6 sigma of the closed form.
+    (H1, n1) < (H2, n2), CSR offsets consistent, and every bucket of Table 2 equal (count and content
+    digest) to the exact match set of the sorted Table 1 (a torch restatement of the match step, itself
+    compared with the oracle's digest mode at K = 27 and on the CPU);
+  * K = 29 and K = 31: 2^13 / 2^12 CONSECUTIVE buckets straight from the oracle (all 2^K nonces hashed).
 Bit-exact: integer work throughout, no tolerance.
 """
 import numpy as np
@@ -385,7 +387,9 @@ def test_K33_full_size_samples_and_properties(vx):
     """BASELINE.json configs[4]: 2^33 nonces, 5-byte nonces, ~512 records per bucket, 174 GB of
     tables on one B200.  Sampled buckets hash by hash against the oracle (5-byte keyed hash) with
     their Table 2 bit-exact; whole-table properties on the device: every nonce exactly once, every
-    partition sorted by (H, n), CSR offsets consistent, |T2| within 6 sigma of the closed form."""
+    partition sorted by (H, n), every stored hash equal to the hash stream (recomputed range by range,
+    itself spot-checked against the oracle), CSR offsets consistent, and EVERY bucket of Table 2 equal in
+    count and content digest to the exact match set of the sorted Table 1."""
     import torch
     K, B = 33, 24
     torch.cuda.empty_cache()
@@ -401,8 +405,6 @@ def test_K33_full_size_samples_and_properties(vx):
     stats = plot.get_stats()
     N = 1 << K
     assert stats["t1_records"] == N
-    mean = N * (1 - 2.0 ** (B - K - 1))
-    assert abs(stats["t2_records"] - mean) < 6 * mean ** 0.5 + 8
     rng = np.random.default_rng(33)
     starts = [0, (1 << 24) - 4] + [int(x) for x in rng.integers(0, (1 << 24) - 4, 14)]
     n = check_sampled_buckets(plot, K, key, [(s, s + 4) for s in starts])
@@ -423,9 +425,18 @@ def test_K33_full_size_samples_and_properties(vx):
     lane = torch.arange(cap, device=dev)[None, :]
     chunk = (1 << 25) // cap
     lowmask = (1 << pbits) - 1
-    R = 1 << 30                                          # nonce range checked per pass
+    # per pass over Table 1: a nonce range of R nonces, its hash stream recomputed by vx_hash_range
+    # (the 68 GB stream of all 2^33 hashes does not fit beside the tables)
+    free, _ = torch.cuda.mem_get_info()
+    R = 1 << 30 if free > (14 << 30) else 1 << 29 if free > (8 << 30) else 1 << 28
+    rng = np.random.default_rng(33)
     for r0 in range(0, N, R):
         seen = torch.zeros(R, dtype=torch.bool, device=dev)
+        hashes = plot.hash_range(r0, R)
+        pick = np.unique(rng.integers(0, R, 1 << 13))     # the stream against the oracle, 5-byte nonces
+        got = hashes[torch.from_numpy(pick).to(dev)].cpu().numpy().view(np.uint64)
+        want = np.array([oracle.hash_nonce(key, int(r0 + n), 5) for n in pick], dtype=np.uint64)
+        assert np.array_equal(got, want), "the hash stream differs from the oracle"
         for p0 in range(0, P, chunk):
             ak = a[p0:p0 + chunk]
             valid = lane < cnt[p0:p0 + chunk, None]
@@ -438,10 +449,17 @@ def test_K33_full_size_samples_and_properties(vx):
                 del k, ok
             non = ((ak & lowmask) << plot.tile_log) | bk
             sel = valid & (non >= r0) & (non < r0 + R)
-            seen[non[sel] - r0] = True
-            del ak, valid, bk, non, sel
+            idx = non[sel] - r0
+            seen[idx] = True
+            # the stored hash (partition index = its top pb bits, a >> pb = the rest) is the nonce's hash
+            pid = torch.arange(p0, p0 + ak.shape[0], device=dev)[:, None].expand_as(ak)
+            Hrec = (pid[sel] << (64 - pbits)) | t_lsr(ak[sel], pbits)
+            assert bool((hashes[idx] == Hrec).all()), "a stored hash differs from the hash stream"
+            del ak, valid, bk, non, sel, idx, pid, Hrec
         assert int(seen.sum()) == R, "some nonce is missing from Table 1 (or appears twice)"
-        del seen
+        del seen, hashes
+    # Table 2, every bucket: count and content digest against the exact match set of the sorted Table 1
+    whole_table2_digest_check(plot, K)
     plot.free()
 
 
