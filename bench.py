@@ -40,10 +40,28 @@ BUCKET_BITS = 24
 ALU_OPS_PER_NONCE = 415            # xor / rotate / byte-swap lane-ops that need the ALU pipe
 S2_BYTES_PER_NONCE = 12 + 12 + 8   # read record, write sorted record, write ~1 Table-2 record
 S1_BYTES_PER_NONCE = 12            # write the record once
-# DRAM bytes per nonce measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one
-# launch at K=29 / 2^29; profiles/r01_final3.md) -- the same kernels and tile geometry at every K
-S1_DRAM_BYTES_PER_NONCE_NCU = 21.9
-S2_DRAM_BYTES_PER_NONCE_NCU = 40.3
+# integer ALU pipe: warp instructions issue at one per 2 clocks per SM sub-partition = 16 lanes/clk, measured
+# with dependent-free LOP3 / SHF chains (bench.py --probe-alu; profiles/r02_alu_probe.md)
+ALU_LANES_PER_SMSP = 16
+# roofline.traffic: DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per nonce of one launch
+# from an ncu --set full capture of THIS tree's kernels, per kernel geometry (layout, tile_log); the
+# bytes per nonce depend on the geometry, not on K.  Each entry names the file under profiles/ it was
+# read from; a geometry with no capture reports traffic = null rather than another geometry's number.
+NCU_TRAFFIC = {
+    # (layout, tile_log): {"s1": B/nonce of vx_k_hash_scatter (+ vx_k_compact in the wide layout),
+    #                      "s2": B/nonce of vx_k_sort_match, "source": file}
+}
+
+
+def load_ncu_traffic():
+    """profiles/r02_traffic.json: written from the round's ncu captures (see profiles/r02_ncu.md)."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        with open(path) as f:
+            for row in json.load(f)["geometries"]:
+                NCU_TRAFFIC[(row["layout"], int(row["tile_log"]))] = row
+    except Exception:
+        pass
 
 
 def measured_peaks():
@@ -155,12 +173,63 @@ def oracle_plot_seconds(K: int, seed: int):
     return t2 - t0, t1 - t0, t2 - t1, len(n1)
 
 
-def cpu_baseline(sample_K: int):
-    total, s1, s2, m = oracle_plot_seconds(sample_K, sample_K)
-    return {"value": (1 << sample_K) / total, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"whole plot at K={sample_K} (2^{sample_K} nonces, key SplitMix64({sample_K}), B=24), "
-                      f"single thread: Table 1 {s1:.2f} s + Table 2 {s2:.2f} s, |T2|={m}",
-            "seconds": total}
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_plot_parallel_hash(K: int, seed: int, workers: int):
+    """One whole plot with the oracle, the hashing shared by `workers` threads, each running the
+    single-threaded C loop on its own nonce range (ctypes releases the GIL; the oracle keeps no global
+    state); bucketing, sorting and matching on one thread.  (seconds hash, bucket+sort, match, |T2|)."""
+    import numpy as np
+    import oracle
+    import vx_inputs
+    key = vx_inputs.key_from_seed(seed)
+    N = 1 << K
+    t0 = time.perf_counter()
+    H = oracle.hash_range_parallel(key, oracle.nonce_size(K), 0, N, workers)
+    t1 = time.perf_counter()
+    off, non, has = oracle.table1_from_records(BUCKET_BITS, 0, 1 << BUCKET_BITS, np.arange(N, dtype=np.uint64), H)
+    t2 = time.perf_counter()
+    t2o, n1, n2 = oracle.table2(K, off, non, has, 1)
+    t3 = time.perf_counter()
+    return t1 - t0, t2 - t1, t3 - t2, len(n1)
+
+
+def cpu_baseline(full_K: int):
+    """BASELINE.md section 4 / SURVEY 8(d): the oracle as it stands (gcc -O2, no intrinsics) on this box's
+    host cores: K=20 in full on one thread, per stage; K=`full_K` (27) in full, per stage, the hashing
+    as P = nproc single-threaded workers over disjoint nonce ranges; K=31 extrapolated from the measured
+    K=27 rates and labelled so."""
+    P = os.cpu_count() or 1
+    t20, s1_20, s2_20, m20 = oracle_plot_seconds(20, 1)
+    h, b, m, nt2 = oracle_plot_parallel_hash(full_K, full_K, P)
+    N = 1 << full_K
+    total = h + b + m
+    per_thread_hash = N / (h * P)
+    rows = [
+        {"K": 20, "threads": 1, "seconds": t20, "table1_s": s1_20, "table2_s": s2_20, "t2_records": m20,
+         "nonces_per_s": (1 << 20) / t20, "kind": "measured, whole plot"},
+        {"K": full_K, "threads": P, "seconds": total, "hash_s": h, "bucket_sort_s": b, "table1_s": h + b,
+         "table2_s": m, "t2_records": nt2, "nonces_per_s": N / total,
+         "hash_nonces_per_s_per_thread": per_thread_hash,
+         "kind": f"measured, whole plot; hashing on {P} threads over disjoint nonce ranges, "
+                 "bucketing + sort + match on one thread"},
+        {"K": 31, "threads": P, "seconds": total * (1 << (31 - full_K)), "nonces_per_s": N / total,
+         "kind": f"extrapolated from the K={full_K} row (x 2^{31 - full_K}); one thread would take about "
+                 f"{(h * P + b + m) * (1 << (31 - full_K)):.0f} s"},
+    ]
+    return {"value": N / total, "unit": UNIT, "cores": P, "kind": "oracle", "cpu": cpu_model(),
+            "sample": f"whole plot at K={full_K} (2^{full_K} nonces, key SplitMix64({full_K}), B=24): hash "
+                      f"{h:.1f} s on {P} threads + bucket/sort {b:.1f} s + match {m:.1f} s on one thread; "
+                      f"K=20 whole plot on one thread {t20:.2f} s",
+            "seconds": total, "single_thread_nonces_per_s": (1 << 20) / t20, "rows": rows}
 
 
 def run_reference(args):
@@ -178,13 +247,19 @@ def run_reference(args):
     value = args.steps * (1 << K) / total
     sample = (f"each step = one whole oracle plot at K={K} (2^{K} nonces, B=24), single thread; "
               f"bounded sample of the K={args.K} workload")
+    ref_config = make_config(args.K)
+    ref_config["workload"] += (f"; REFERENCE ARM: each step is a bounded sample of that workload, one whole oracle "
+                               f"plot at K={K} (2^{K} nonces, key SplitMix64({K}), B=24) on one host thread -- "
+                               f"value and ms_per_step are the sample's, not a K={args.K} plot's")
+    ref_config["reference_sample_K"] = K
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64",
         "data": "synthetic", "gpu_launches": 0,
-        "config": make_config(args.K),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "config": ref_config,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "cpu": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
@@ -218,7 +293,7 @@ def run_cuda(args):
     K = args.K
     # independent plots: rank r plots under key SplitMix64(seed_for_K + 1000 r)
     key = vx_inputs.key_from_seed(rank_seed(K, rank))
-    plot = vx.Plot(K, key, BUCKET_BITS, device=dev)
+    plot = vx.Plot(K, key, BUCKET_BITS, device=dev, flags=args.flags)
     N = 1 << K
     stream = torch.cuda.current_stream()
 
@@ -243,7 +318,19 @@ def run_cuda(args):
     for i in range(args.steps):
         step(evs[i])
     barrier()
+    # a short run (small K) ends before nvidia-smi has printed a line: keep the same workload running,
+    # untimed, until there are three samples, and say so
+    extra = 0
+    if rank == 0:
+        t_end = time.perf_counter() + 3.0
+        while len(sampler.rows) < 3 and time.perf_counter() < t_end:
+            step(); extra += 1
+            torch.cuda.synchronize()
     clocks = sampler.stop() if rank == 0 else None
+    if clocks is not None:
+        clocks["sampled_during"] = ("the timed region" if extra == 0 else
+                                    f"the timed region + {extra} untimed steps of the same workload right behind it")
+    barrier()
     total_ms = evs[0][0].elapsed_time(evs[-1][2])
     s1_ms = [e[0].elapsed_time(e[1]) for e in evs]
     s2_ms = [e[1].elapsed_time(e[2]) for e in evs]
@@ -252,7 +339,7 @@ def run_cuda(args):
     # ---- end to end through the C ABI with host buffers -----------------------------------
     # per step: key (32 B) in; Table 2 + its offsets out, streamed through a pinned staging buffer
     nb = 1 << BUCKET_BITS
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    e2e_steps = max(1, args.e2e_steps if args.e2e_steps > 0 else args.steps)
     d2h = 0
     streamed = not args.e2e_serial
     if streamed:
@@ -276,7 +363,7 @@ def run_cuda(args):
 
         def e2e_step():
             nonlocal d2h
-            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace)  # key -> kernel params
+            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace, flags=args.flags)  # key -> kernel params
             p2.build_table1(stream)
             d2h = p2.sort_match_table2_to_host(copy_stream, pinned_rec.data_ptr(), rec_cap, pinned_off.data_ptr(),
                                                slices=args.e2e_slices, stream=stream) + (nb + 1) * 8
@@ -293,7 +380,7 @@ def run_cuda(args):
 
         def e2e_step():
             nonlocal d2h
-            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace)  # key -> kernel params
+            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace, flags=args.flags)  # key -> kernel params
             p2.build_table1(stream)
             p2.sort_match_table2(stream)
             moved = 0
@@ -339,19 +426,24 @@ def run_cuda(args):
 
     if rank == 0:
         peaks = measured_peaks()
-        alu_peak = 148 * 4 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12     # T lane-ops/s on the ALU pipe
+        load_ncu_traffic()
+        geom = ("wide" if plot.wide else "narrow", plot.tile_log)
+        tr = NCU_TRAFFIC.get(geom)
+        alu_peak = 148 * 4 * ALU_LANES_PER_SMSP * peaks["sm_max_mhz"] * 1e6 / 1e12     # T lane-ops/s on the ALU pipe
         r1 = {"kernel": "vx_k_hash_scatter", "bound": "alu", "achieved": ALU_OPS_PER_NONCE * N / (s1 * 1e-3) / 1e12,
-              "peak": alu_peak, "unit": "Tlaneop/s", "traffic": S1_DRAM_BYTES_PER_NONCE_NCU * N, "ms": s1,
+              "peak": alu_peak, "unit": "Tlaneop/s", "traffic": tr["s1"] * N if tr else None, "ms": s1,
               "hbm_algorithmic_GBps": S1_BYTES_PER_NONCE * N / (s1 * 1e-3) / 1e9}
         r1["frac"] = r1["achieved"] / r1["peak"]
         r2 = {"kernel": "vx_k_sort_match", "bound": "hbm", "achieved": S2_BYTES_PER_NONCE * N / (s2 * 1e-3) / 1e9,
-              "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": S2_DRAM_BYTES_PER_NONCE_NCU * N, "ms": s2}
+              "peak": peaks["hbm_gbs"], "unit": "GB/s", "traffic": tr["s2"] * N if tr else None, "ms": s2}
         r2["frac"] = r2["achieved"] / r2["peak"]
         dominant = dict(r1 if s1 >= s2 else r2)
-        dominant["traffic_source"] = ("ncu --set full at K=29 (profiles/r01_final3.md): DRAM read+write bytes per "
-                                      "nonce of this kernel x 2^K")
-        dominant["peak_source"] = peaks["source"] + (" (hbm_gbs, burst copy)" if dominant["bound"] == "hbm"
-                                                     else " (sm_max_mhz x 148 SM x 4 SMSP x 16 ALU lanes; DESIGN.md)")
+        dominant["traffic_source"] = (f"{tr['source']}: DRAM read+write bytes per nonce of this kernel in the "
+                                      f"{geom[0]} layout with 2^{geom[1]}-record tiles x 2^K" if tr else
+                                      f"no ncu capture of the {geom[0]} layout with 2^{geom[1]}-record tiles")
+        dominant["peak_source"] = peaks["source"] + (" (hbm_gbs, burst copy)" if dominant["bound"] == "hbm" else
+                                                     f" (sm_max_mhz) x 148 SM x 4 SMSP x {ALU_LANES_PER_SMSP} ALU lanes/clk: "
+                                                     "profiles/r02_alu_probe.md (bench.py --probe-alu)")
         line = {
             "metric": METRIC, "value": whole_job_value(K, world, ms_per_step), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
@@ -376,6 +468,42 @@ def run_cuda(args):
     plot.free()
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def run_probe_alu(args):
+    """Issue rate of the integer pipes: dependent-free chains of one instruction kind, 2048 threads per
+    SM, timed with CUDA events; lane-ops per clock per SM at the SM clock sampled during the run."""
+    import torch
+
+    import paper_2606_14007_b200 as vx
+    torch.cuda.set_device(0)
+    scratch = torch.zeros(1024, dtype=torch.int32, device="cuda:0")
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    iters = 1 << 14
+    out = {}
+    sampler = ClockSampler(0)
+    sampler.start()
+    for kind in ("lop3", "shf", "arx", "prmt", "add", "imad"):
+        for _ in range(2):
+            vx.probe_alu(kind, iters, scratch)
+        torch.cuda.synchronize()
+        best = None
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ops = vx.probe_alu(kind, iters, scratch)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        out[kind] = {"lane_ops": ops, "ms": best, "Tlaneop_per_s": ops / (best * 1e-3) / 1e12}
+    clocks = sampler.stop()
+    mhz = clocks.get("sm_mhz") or measured_peaks()["sm_max_mhz"]
+    for v in out.values():
+        v["lanes_per_clk_per_sm"] = v["Tlaneop_per_s"] * 1e12 / (mhz * 1e6) / sms
+        v["lanes_per_clk_per_smsp"] = v["lanes_per_clk_per_sm"] / 4
+    print(json.dumps({"probe": "alu", "sms": sms, "sm_mhz": mhz, "clocks": clocks, "kinds": out}), flush=True)
     return 0
 
 
@@ -428,9 +556,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--K", type=int, default=31, help="plot size; 31 = the configuration the metric is quoted on")
-    ap.add_argument("--cpu-K", dest="cpu_K", type=int, default=24, help="oracle sample size for cpu_baseline")
+    ap.add_argument("--cpu-K", dest="cpu_K", type=int, default=27,
+                    help="cpu_baseline: the oracle makes this plot in full (hashing on nproc threads), and K=20 on one")
+    ap.add_argument("--flags", type=int, default=0,
+                    help="test-only layout flags (1 wide layout, 2 big tiles): ncu captures of the K>=32 geometries at small K")
+    ap.add_argument("--probe-alu", dest="probe_alu", action="store_true",
+                    help="integer-pipe issue rates from dependent-free instruction chains (vx_probe_alu), one JSON line")
     ap.add_argument("--ref-K", dest="ref_K", type=int, default=22, help="oracle sample size per --impl reference step")
-    ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=0, help="0 = as many as --steps")
     ap.add_argument("--e2e-chunks", dest="e2e_chunks", type=int, default=32)
     ap.add_argument("--e2e-slices", dest="e2e_slices", type=int, default=64)
     ap.add_argument("--e2e-inflight", dest="e2e_inflight", type=int, default=2,
@@ -443,6 +576,8 @@ def main():
         print("bench.py: note: warmup < 3 breaks the timing rules", file=sys.stderr)
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe_alu:
+        return run_probe_alu(args)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.gpus != world:
         if world == 1 and args.gpus > 1:

@@ -171,9 +171,9 @@ vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64
  * synchronising call instead of dropping records silently (reading A8). */
 #define VX_OPT_PARTITION_CAPACITY_LIMIT 2
 #define VX_OPT_TABLE2_CAPACITY_LIMIT 3
-/* VX_OPT_SUBKEY_BITS (0 .. 32, default 32): how many hash bits below the bin index the fused kernel's
- * fast in-bin ranking compares.  Fewer bits make records of one bin tie, come out in the wrong order
- * and so send the tile through its "redo with exact (H, n) ranks" path (taken about once per 2^21
+/* VX_OPT_SUBKEY_BITS (0 .. 32, default 32; 31 and above mean all 31 the kernel keeps): how many hash
+ * bits below the bin index the fused kernel's fast in-bin ranking compares.  Fewer bits make records of one bin tie, come out in the wrong order
+ * and so send the tile through its "redo with exact (H, n) ranks" path (taken about once per 2^20
  * tiles otherwise) -- results are identical by construction; tests use it to run that path. */
 #define VX_OPT_SUBKEY_BITS 4
 vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value);

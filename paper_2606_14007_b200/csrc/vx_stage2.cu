@@ -145,12 +145,13 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
     return excl;
 }
 
-// the 32 hash bits right below the bin index (bin = (H >> binshift) & (VX_NBINS - 1))
-// binshift >= 32 always (pb + VX_BIN_BITS <= 32; checked at launch), so both are 32-bit operations on
-// the high word: sh = binshift - 32
+// the 31 hash bits right below the bin index (bin = (H >> binshift) & (VX_NBINS - 1)), as a value
+// below 2^31 (so that sub-key + 1 never wraps, see the ranking pass).  binshift >= 32 always
+// (pb + VX_BIN_BITS <= 32; checked at launch), so both are 32-bit operations on the high word:
+// sh = binshift - 32
 __device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int sh)
 {
-    return __funnelshift_r((uint32_t)k, (uint32_t)(k >> 32), sh);
+    return __funnelshift_r((uint32_t)k, (uint32_t)(k >> 32), sh) >> 1;
 }
 template <uint32_t NBINS>
 __device__ __forceinline__ uint32_t vx_bin(uint64_t k, int sh)
@@ -252,7 +253,27 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
     for (;;) {
         __syncthreads();                                // previous tile fully drained
-        if (tid == 0) s_tile = q.tile_begin + atomicAdd(&q.ctrl->ticket, 1u);
+        if (tid == 0) {
+            const uint32_t t = q.tile_begin + atomicAdd(&q.ctrl->ticket, 1u);
+            s_tile = t;
+            // Tickets are handed out in partition order and the CTAs run about one tile apart, so the
+            // partition gridDim tickets ahead is the one some CTA (most likely this one) takes next:
+            // one bulk prefetch (TMA, cp.async.bulk.prefetch.L2 -> UBLKPF.L2) brings its 64 KB into
+            // L2 while this tile is sorted, and phase A's loads no longer wait for HBM (K=31:
+            // 33.9 -> 32.7 ms).  A hint only: nothing depends on who takes that partition, or when.
+            const uint32_t pf = t + gridDim.x;
+            if (pf < q.tile_end) {
+                const uint32_t n = min(q.cursor[pf], q.cap_check);
+                const char *p = reinterpret_cast<const char *>(q.part) + (size_t)pf * q.cap * (WIDE ? 8 : 16);
+                const uint32_t bytes = n * (WIDE ? 8u : 16u) & ~15u;
+                if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(p), "r"(bytes) : "memory");
+                if constexpr (WIDE) {
+                    const char *pb2 = reinterpret_cast<const char *>(q.part_b) + (size_t)pf * q.cap * 2;
+                    const uint32_t b2 = n * 2u & ~15u;
+                    if (b2) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(pb2), "r"(b2) : "memory");
+                }
+            }
+        }
         // exact = rank by (H, n) with full compares; the fast pass ranks by H alone and is
         // validated in phase E (a tile holding two equal hashes comes back for an exact pass)
         uint32_t exact = q.force_exact | (q.do_match ^ 1u);
@@ -355,18 +376,20 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         // with equal sub-keys (or equal hashes) may come out in the wrong order, which
                         // phase E sees as keys that do not strictly increase
                         const uint32_t *sp = sub + s;
-                        const uint32_t ks = vx_subkey(k, sh) & submask;
+                        const uint32_t ks = sub[i];                         // < 2^31
                         const uint32_t me = i - s;
+                        // (kj, j) < (ks, me)  <=>  kj < ks + (j < me); the own slot and the slots
+                        // beyond the bin (sentinel ~0) never count
 #pragma unroll
                         for (uint32_t j = 0; j < 4; j++) {
                             const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
-                            rank += (kj < ks || (kj == ks && j < me)) ? 1u : 0u;
+                            rank += kj < ks + (j < me ? 1u : 0u) ? 1u : 0u;
                         }
                         if (nm > 4) {
 #pragma unroll 1
                             for (uint32_t j = 4; j < nm; j++) {
                                 const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
-                                rank += (kj < ks || (kj == ks && j < me)) ? 1u : 0u;
+                                rank += kj < ks + (j < me ? 1u : 0u) ? 1u : 0u;
                             }
                         }
                     } else {                            // by (H, n), reading A10
@@ -659,7 +682,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.cap_check = g.cap_check; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
-    q.submask = g.subkey_bits >= 32 ? ~0u : g.subkey_bits == 0 ? 0u : ~0u << (32 - g.subkey_bits);
+    q.submask = g.subkey_bits >= 31 ? 0x7fffffffu : (0x7fffffffu >> (31 - g.subkey_bits)) << (31 - g.subkey_bits);
     q.tile_begin = tile_begin; q.tile_end = tile_end; q.slice_end_out = slice_end_out;
     if (g.pb + g.tile_log > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
     q.part_b = (uint16_t *)(ws + g.off_part_b);
@@ -683,6 +706,9 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.nlo_bits = g.tile_log;
     const bool big = g.tile_log == VX_TILE_LOG_BIG;
     uint64_t grid = (uint64_t)num_sms * (big ? 1 : VX_S2_MINB);
+#ifdef VX_EXP_GRID_PER_SM
+    grid = (uint64_t)num_sms * VX_EXP_GRID_PER_SM;      // experiment: CTAs per SM
+#endif
     if (grid > tile_end - tile_begin) grid = tile_end - tile_begin;
     if (big && g.wide) VX_S2B_KERNEL(true)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
     else if (big) VX_S2B_KERNEL(false)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
