@@ -65,9 +65,12 @@ size_t vx_workspace_bytes(uint32_t K);
 /* Same for a test-only bucket_bits (see vx_plot_create_ex). */
 size_t vx_workspace_bytes_ex(uint32_t K, uint32_t bucket_bits);
 
-/* Create a plot handle for 2^K nonces under a 256-bit key (host pointer, copied).  K in 1..33 with
- * 2^24 buckets (mean bucket <= 512 records, BASELINE.json's K=33); K = 33 uses 5-byte nonces
- * (reading A1) and the compact "wide" internal layout below.  PAPER.md L41-43. */
+/* Create a plot handle for 2^K nonces under a 256-bit key (host pointer, copied).  K in 1..36 with
+ * 2^24 buckets; K >= 33 uses 5-byte nonces (reading A1) and the compact "wide" internal layout
+ * below.  Up to K = 33 (BASELINE.json's largest configuration, mean bucket 512 records, 171 GB) the
+ * whole plot is resident at once; K = 34..36 is made in 2^(K-33) bucket-range PASSES (below), each
+ * the size of a K = 33 plot.  (SURVEY.md 8(b) allowed K up to 40: beyond 36 the packed Table-2 record
+ * of the wide layout, 4 high nonce bits per nonce, would have to grow.)  PAPER.md L41-43. */
 vx_status vx_plot_create(uint32_t K, const uint8_t key[32], vx_plot **out);
 /* Test-only: bucket_bits B in 1..24 instead of 24 (dense buckets at tiny K, reading A7). */
 vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, vx_plot **out);
@@ -78,6 +81,12 @@ vx_status vx_plot_create_ex(uint32_t K, const uint8_t key[32], uint32_t bucket_b
 /* VX_CREATE_BIG_TILES: use the K >= 32 tile geometry (2^13-record partitions, one 1024-thread CTA
  * per SM) at this K, for the same reason. */
 #define VX_CREATE_BIG_TILES 2u
+/* VX_CREATE_PASSES_LOG(l): make the plot in 2^l bucket-range passes (l in 1..8; l <= partition bits)
+ * whatever K is -- the test-only "VRAM budget" with which the multi-pass path is compared with the
+ * oracle on small tables.  Without it K <= 33 takes one pass and K >= 34 the fewest that fit. */
+#define VX_CREATE_PASSES_LOG_SHIFT 8
+#define VX_CREATE_PASSES_LOG_MASK 0xf00u
+#define VX_CREATE_PASSES_LOG(l) ((uint32_t)(l) << VX_CREATE_PASSES_LOG_SHIFT)
 vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket_bits, uint32_t flags,
                               vx_plot **out);
 size_t vx_workspace_bytes_opts(uint32_t K, uint32_t bucket_bits, uint32_t flags);
@@ -127,6 +136,30 @@ vx_status vx_sort_match_table2_to_host(vx_plot *p, void *compute_stream, void *c
                                        size_t *records_bytes);
 vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
                                        int fd, void *pinned_staging, size_t staging_bytes, uint64_t *file_bytes);
+
+/* Bucket-range passes (VI: "chunked VRAM tiling to handle k > 31
+ * without requiring the full Table-1 in VRAM").  A plot with P = 2^l passes is made one hash-prefix
+ * slice at a time: pass s hashes ALL 2^K nonces but keeps only the records whose top l hash bits are
+ * s, i.e. the buckets [s 2^B / P, (s + 1) 2^B / P); Table 1, Table 2 and their offsets of that slice
+ * occupy the workspace (sized for one pass) until the next pass is selected.  The buckets of
+ * different passes are disjoint and complete, so the passes together are exactly the one-pass plot.
+ *   vx_plot_passes       P, the selected pass and its bucket range (any pointer may be NULL);
+ *   vx_plot_select_pass  choose the slice that vx_build_table1 / vx_sort_match_table2* / vx_read_tables
+ *                        / vx_get_stats act on (default 0; reads outside its bucket range return
+ *                        VX_ERR_RANGE; vx_get_stats counts the slice).  Synchronises; the previous
+ *                        slice's tables are gone afterwards;
+ *   vx_plot_all_passes_to_host  the whole plot: for every pass, vx_build_table1 and the streamed egress
+ *                        of vx_sort_match_table2_to_host, Table 2 appended to host_records (HOST,
+ *                        records_capacity bytes) and the CSR offsets of all 2^B buckets (global, in
+ *                        records) written to host_offsets (HOST, 2^B + 1 entries, may be NULL).
+ *                        *records_bytes = bytes written, *t1_records = records placed over all passes
+ *                        (= 2^K).  Blocks.  One pass: the same as build + _to_host. */
+vx_status vx_plot_passes(const vx_plot *p, uint32_t *passes, uint32_t *selected, uint64_t *bucket_begin,
+                         uint64_t *bucket_end);
+vx_status vx_plot_select_pass(vx_plot *p, uint32_t pass);
+vx_status vx_plot_all_passes_to_host(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                                     void *host_records, size_t records_capacity, uint64_t *host_offsets,
+                                     size_t *records_bytes, uint64_t *t1_records);
 
 /* Copy the buckets [bucket_begin, bucket_end) of table 1 or 2 to HOST memory in the external
  * format.  Synchronises the plot's stream.  offsets_out (may be NULL) receives

@@ -20,6 +20,11 @@ VX_OPT_TABLE2_CAPACITY_LIMIT = 3
 VX_OPT_SUBKEY_BITS = 4
 VX_CREATE_WIDE_LAYOUT = 1
 VX_CREATE_BIG_TILES = 2
+
+
+def VX_CREATE_PASSES_LOG(l: int) -> int:
+    return l << 8
+
 STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPACE", -4: "VX_ERR_CUDA",
           -5: "VX_ERR_OVERFLOW", -6: "VX_ERR_RANGE", -7: "VX_ERR_UNSUPPORTED", -8: "VX_ERR_IO", -9: "VX_ERR_NOMEM"}
 
@@ -27,7 +32,8 @@ STATUS = {0: "VX_OK", -1: "VX_ERR_ARG", -2: "VX_ERR_STATE", -3: "VX_ERR_WORKSPAC
 EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_opts", "vx_plot_create",
            "vx_plot_create_ex", "vx_plot_create_opts",
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
-           "vx_sort_match_table2_to_file", "vx_read_tables",
+           "vx_sort_match_table2_to_file", "vx_read_tables", "vx_plot_passes", "vx_plot_select_pass",
+           "vx_plot_all_passes_to_host",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink", "vx_probe_alu",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
@@ -86,6 +92,14 @@ def load_library() -> ctypes.CDLL:
     L.vx_sort_match_table2_to_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _sz, _vp, ctypes.POINTER(_sz)]
     L.vx_sort_match_table2_to_file.restype = ctypes.c_int
     L.vx_sort_match_table2_to_file.argtypes = [_vp, _vp, _vp, _u32, ctypes.c_int, _vp, _sz, ctypes.POINTER(_u64)]
+    L.vx_plot_passes.restype = ctypes.c_int
+    L.vx_plot_passes.argtypes = [_vp, ctypes.POINTER(_u32), ctypes.POINTER(_u32), ctypes.POINTER(_u64),
+                                 ctypes.POINTER(_u64)]
+    L.vx_plot_select_pass.restype = ctypes.c_int
+    L.vx_plot_select_pass.argtypes = [_vp, _u32]
+    L.vx_plot_all_passes_to_host.restype = ctypes.c_int
+    L.vx_plot_all_passes_to_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _sz, _vp, ctypes.POINTER(_sz),
+                                             ctypes.POINTER(_u64)]
     L.vx_read_tables.restype = ctypes.c_int
     L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
     L.vx_device_tables.restype = ctypes.c_int
@@ -158,6 +172,9 @@ class Plot:
         l1, l2 = _u32(), _u32()
         self._L.vx_plot_launches(self._h, ctypes.byref(l1), ctypes.byref(l2))
         self.launches_per_plot = l1.value + l2.value
+        np_, sel = _u32(), _u32()
+        self._L.vx_plot_passes(self._h, ctypes.byref(np_), ctypes.byref(sel), None, None)
+        self.passes = np_.value
         self.rec1_bytes = self.nonce_size + 8
         self.rec2_bytes = 2 * self.nonce_size
         need = int(self._L.vx_workspace_bytes_opts(K, bucket_bits, flags))
@@ -233,6 +250,26 @@ class Plot:
                 ctypes.byref(n)))
         return n.value
 
+    def select_pass(self, s: int):
+        with self._dev():
+            self._check(self._L.vx_plot_select_pass(self._h, s))
+
+    def pass_buckets(self):
+        """(bucket_begin, bucket_end) of the selected pass."""
+        b0, b1 = _u64(), _u64()
+        self._L.vx_plot_passes(self._h, None, None, ctypes.byref(b0), ctypes.byref(b1))
+        return b0.value, b1.value
+
+    def all_passes_to_host(self, copy_stream, records_ptr: int, records_capacity: int, offsets_ptr: int = 0,
+                           slices: int = 16, stream=None):
+        """The whole plot, pass by pass, Table 2 streamed to host memory: (record bytes, Table-1 records)."""
+        need, t1 = _sz(), _u64()
+        with self._dev():
+            self._check(self._L.vx_plot_all_passes_to_host(
+                self._h, self._sp(stream), self._sp(copy_stream), slices, records_ptr, records_capacity,
+                offsets_ptr or None, ctypes.byref(need), ctypes.byref(t1)))
+        return need.value, t1.value
+
     def synchronize(self):
         with self._dev():
             self._check(self._L.vx_synchronize(self._h))
@@ -249,11 +286,14 @@ class Plot:
             self._check(self._L.vx_get_counters(self._h, ctypes.byref(r)))
         return {"tile_retries": r.value}
 
-    def read_tables(self, table: int, bucket_begin: int = 0, bucket_end: int | None = None,
+    def read_tables(self, table: int, bucket_begin: int | None = None, bucket_end: int | None = None,
                     records_out: np.ndarray | None = None):
-        """(offsets uint64[nb+1] relative to the range, records uint8[...]) copied to the host."""
+        """(offsets uint64[nb+1] relative to the range, records uint8[...]) copied to the host.
+        Default range: all buckets of the selected pass (= all 2^B buckets of a one-pass plot)."""
+        if bucket_begin is None:
+            bucket_begin = self.pass_buckets()[0]
         if bucket_end is None:
-            bucket_end = 1 << self.bucket_bits
+            bucket_end = self.pass_buckets()[1]
         nb = bucket_end - bucket_begin
         offsets = np.empty(max(nb, 0) + 1, dtype=np.uint64)
         need = _sz()

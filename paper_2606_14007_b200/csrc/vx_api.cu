@@ -32,11 +32,19 @@ struct vx_plot {
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // ------------------------------------------------------------------------------ geometry
-bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles)
+void vx_geom_select_pass(VxGeom *g, uint32_t pass)
+{
+    g->pass = pass;
+    g->p_first = (uint64_t)pass * g->P;
+    g->b_first = (uint64_t)pass * g->NBp;
+}
+
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles, uint32_t passes_log)
 {
     memset(g, 0, sizeof *g);
-    if (K < 1 || K > 36 || B < 1 || B > 24) return false;  // wide Table-2 records keep 4 high nonce bits
-    if (K > B + VX_MAX_MEAN_BUCKET_LOG) return false;
+    if (K < 1 || K > VX_MAX_K || B < 1 || B > 24) return false;
+    if (passes_log > VX_MAX_PASSES_LOG) return false;
+    if (K > B + VX_MAX_MEAN_BUCKET_LOG + passes_log) return false;
     g->K = K; g->B = B;
     g->nonce_size = K <= 32 ? 4 : 5;                       // reading A1
     g->wide = (g->nonce_size > 4 || force_wide) ? 1u : 0u;
@@ -44,7 +52,11 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     g->pb = K > g->tile_log ? K - g->tile_log : 0;
     if (g->pb > B) return false;                           // cannot happen while K - B <= 9
     g->fb = B - g->pb;
-    g->N = 1ull << K; g->P = 1ull << g->pb; g->NB = 1ull << B;
+    if (passes_log > g->pb || passes_log > B) return false;  // a pass is a whole number of partitions (and buckets)
+    g->passes_log = passes_log;
+    g->N = 1ull << K; g->P = 1ull << (g->pb - passes_log); g->NB = 1ull << B;
+    g->NBp = g->NB >> passes_log;
+    vx_geom_select_pass(g, 0);
     const uint64_t mean = g->N >> g->pb;
     uint64_t cap;
     if (g->pb == 0) cap = mean;                            // the single partition holds everything
@@ -54,7 +66,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     g->cap = (uint32_t)cap;
     g->cap_check = g->cap;
     // |T2| ~ 2^K (1 - 2^(B-K-1)) for K >= B, 2^(2K-1-B) below; sd ~ sqrt: 2^K + slack is ample
-    g->t2_cap = g->N + (1u << 16);
+    g->t2_cap = (g->N >> passes_log) + (1u << 16);        // per pass
     g->t2_check = g->t2_cap;
     g->subkey_bits = 32;
     g->rec1_bytes = g->nonce_size + 8;
@@ -70,8 +82,8 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
         g->off_part = o;   o = align256(o + g->P * (size_t)g->cap * 8);
         g->off_part_b = o; o = align256(o + g->P * (size_t)g->cap * 2);
     }
-    g->off_t1_off = o;    o = align256(o + (g->NB + 1) * 8);
-    g->off_t2_off = o;    o = align256(o + (g->NB + 1) * 8);
+    g->off_t1_off = o;    o = align256(o + (g->NBp + 1) * 8);
+    g->off_t2_off = o;    o = align256(o + (g->NBp + 1) * 8);
     size_t t2_bytes = g->t2_cap * (size_t)8;
     if (g->wide) {
         // stage 1 in rounds: 4 slices (K >= 2), scratch partitions one hash bit coarser than the
@@ -79,20 +91,20 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
         // the geometry stage 1 runs ALU-bound in at K = 31.
         g->round_log = K >= 2 ? K - 2 : K;
         g->rounds = 1u << (K - g->round_log);
-        g->pb_tmp = g->pb ? g->pb - 1 : 0;
+        g->pb_tmp = g->pb > passes_log ? g->pb - 1 : g->pb;     // (global bit count, like pb)
         const uint64_t mean_tmp = (1ull << g->round_log) >> g->pb_tmp;
-        uint64_t cap_tmp = g->pb_tmp == 0 ? mean_tmp : mean_tmp + (uint64_t)ceil(8.0 * sqrt((double)mean_tmp));
+        uint64_t cap_tmp = (g->pb_tmp == 0 && passes_log == 0) ? mean_tmp : mean_tmp + (uint64_t)ceil(8.0 * sqrt((double)mean_tmp));
         cap_tmp = (cap_tmp + 31) & ~(uint64_t)31;
         g->cap_tmp = (uint32_t)cap_tmp;
-        const size_t tmp_bytes = ((size_t)1 << g->pb_tmp) * cap_tmp * 16;
+        const size_t tmp_bytes = ((size_t)1 << (g->pb_tmp - passes_log)) * cap_tmp * 16;
         if (tmp_bytes > t2_bytes) t2_bytes = tmp_bytes;      // tiny K only
-        g->off_cursor_tmp = o; o = align256(o + ((size_t)4 << g->pb_tmp));
+        g->off_cursor_tmp = o; o = align256(o + ((size_t)4 << (g->pb_tmp - passes_log)));
     }
     o = (o + ((size_t)2 << 20) - 1) & ~(((size_t)2 << 20) - 1);   // Table 2 on a 2 MB boundary: D2H copies of it run faster aligned
     g->off_t2_rec = o;    o = align256(o + t2_bytes);
     g->off_tmp = g->off_t2_rec;                              // scratch of stage 1, dead before stage 2
     if (g->wide) { g->off_t2_hi = o; o = align256(o + g->t2_cap); }
-    g->stage_bytes = g->N * (size_t)g->rec1_bytes;
+    g->stage_bytes = (g->N >> passes_log) * (size_t)g->rec1_bytes;
     if (g->stage_bytes > VX_STAGE_MAX_BYTES) g->stage_bytes = VX_STAGE_MAX_BYTES;
     g->off_stage = o;     o = align256(o + g->stage_bytes);
     g->total = o;
@@ -191,11 +203,20 @@ const char *vx_status_string(vx_status s)
     return "VX_ERR_?";
 }
 
+// flags -> geometry.  Passes: the explicit VX_CREATE_PASSES_LOG field, else the fewest passes that keep
+// at most 2^33 records resident (K <= 33: one pass).
+static bool geom_from_flags(VxGeom *g, uint32_t K, uint32_t bucket_bits, uint32_t flags)
+{
+    if (flags & ~(uint32_t)(VX_CREATE_WIDE_LAYOUT | VX_CREATE_BIG_TILES | VX_CREATE_PASSES_LOG_MASK)) return false;
+    uint32_t pl = (flags & VX_CREATE_PASSES_LOG_MASK) >> VX_CREATE_PASSES_LOG_SHIFT;
+    if (pl == 0 && K > bucket_bits + VX_MAX_MEAN_BUCKET_LOG && bucket_bits == 24) pl = K - bucket_bits - VX_MAX_MEAN_BUCKET_LOG;
+    return vx_geom_init(g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0, (flags & VX_CREATE_BIG_TILES) != 0, pl);
+}
+
 size_t vx_workspace_bytes_opts(uint32_t K, uint32_t bucket_bits, uint32_t flags)
 {
     VxGeom g;
-    if (flags & ~(uint32_t)(VX_CREATE_WIDE_LAYOUT | VX_CREATE_BIG_TILES)) return 0;
-    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0, (flags & VX_CREATE_BIG_TILES) != 0)) return 0;
+    if (!geom_from_flags(&g, K, bucket_bits, flags)) return 0;
     return g.total;
 }
 
@@ -209,9 +230,8 @@ vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket
     if (!out) return VX_ERR_ARG;
     *out = NULL;
     if (!key) return VX_ERR_ARG;
-    if (flags & ~(uint32_t)(VX_CREATE_WIDE_LAYOUT | VX_CREATE_BIG_TILES)) return VX_ERR_ARG;
     VxGeom g;
-    if (!vx_geom_init(&g, K, bucket_bits, (flags & VX_CREATE_WIDE_LAYOUT) != 0, (flags & VX_CREATE_BIG_TILES) != 0)) return VX_ERR_ARG;
+    if (!geom_from_flags(&g, K, bucket_bits, flags)) return VX_ERR_ARG;
     vx_plot *p = new (std::nothrow) vx_plot;
     if (!p) return VX_ERR_NOMEM;
     memset(p, 0, sizeof *p);
@@ -309,6 +329,10 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
         return fail(p, VX_ERR_STATE, "Table 2 read before vx_sort_match_table2");
     if (bucket_begin > bucket_end || bucket_end > p->g.NB)
         return fail(p, VX_ERR_RANGE, "bucket range outside [0, 2^B]");
+    if (bucket_begin < p->g.b_first || bucket_end > p->g.b_first + p->g.NBp)
+        return fail(p, VX_ERR_RANGE, "bucket range outside the selected pass (vx_plot_select_pass)");
+    bucket_begin -= p->g.b_first;                          // offsets in the workspace are relative to the pass
+    bucket_end -= p->g.b_first;
     if (!p->t1_materialised) {
         // Table 1 read after stage 1 alone: split the partitions into buckets now (no matching)
         cudaError_t e = vx_launch_stage2(p->g, p->ws, false, p->force_exact, p->num_sms, p->stream);
@@ -419,6 +443,8 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
 {
     if (!p) return VX_ERR_ARG;
     if (fd < 0 || !pinned_staging) return fail(p, VX_ERR_ARG, "bad file descriptor or NULL staging buffer");
+    if (p->g.passes_log)
+        return fail(p, VX_ERR_UNSUPPORTED, "the file sink writes one pass; a plot made in passes goes through vx_plot_all_passes_to_host");
     VxRing *ring = vx_ring_create(pinned_staging, staging_bytes, fd);
     if (!ring) return fail(p, VX_ERR_ARG, "staging buffer smaller than two 4 MB chunks");
     uint64_t n = 0;
@@ -436,6 +462,65 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
     }
     if (file_bytes) *file_bytes = written;
     return s;
+}
+
+// ------------------------------------------------------------------------------ passes (8(f3))
+vx_status vx_plot_passes(const vx_plot *p, uint32_t *passes, uint32_t *selected, uint64_t *bucket_begin,
+                         uint64_t *bucket_end)
+{
+    if (!p) return VX_ERR_ARG;
+    if (passes) *passes = 1u << p->g.passes_log;
+    if (selected) *selected = p->g.pass;
+    if (bucket_begin) *bucket_begin = p->g.b_first;
+    if (bucket_end) *bucket_end = p->g.b_first + p->g.NBp;
+    return VX_OK;
+}
+
+vx_status vx_plot_select_pass(vx_plot *p, uint32_t pass)
+{
+    if (!p) return VX_ERR_ARG;
+    if (pass >= (1u << p->g.passes_log)) return fail(p, VX_ERR_ARG, "pass outside [0, passes)");
+    if (p->state >= VX_BUILT) {                            // the workspace is about to be reused
+        vx_status s = sync_and_check(p);
+        if (s != VX_OK) return s;
+    }
+    vx_geom_select_pass(&p->g, pass);
+    if (p->state > VX_BOUND) p->state = VX_BOUND;          // the tables of the other pass are gone
+    p->t1_materialised = false;
+    return VX_OK;
+}
+
+vx_status vx_plot_all_passes_to_host(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
+                                     void *host_records, size_t records_capacity, uint64_t *host_offsets,
+                                     size_t *records_bytes, uint64_t *t1_records)
+{
+    if (!p) return VX_ERR_ARG;
+    if (!host_records) return fail(p, VX_ERR_ARG, "NULL host_records");
+    if (p->state < VX_BOUND) return fail(p, VX_ERR_STATE, "vx_plot_all_passes_to_host before vx_plot_bind");
+    const uint32_t passes = 1u << p->g.passes_log;
+    const size_t rb = p->g.rec2_bytes;
+    uint64_t total = 0, t1_total = 0;
+    if (records_bytes) *records_bytes = 0;
+    for (uint32_t s = 0; s < passes; s++) {
+        vx_status st = vx_plot_select_pass(p, s);
+        if (st == VX_OK) st = vx_build_table1(p, compute_stream);
+        if (st != VX_OK) return st;
+        uint64_t n = 0;
+        uint64_t *off = host_offsets ? host_offsets + p->g.b_first : NULL;
+        st = egress_common(p, compute_stream, copy_stream, slices, (uint8_t *)host_records + total * rb,
+                           records_capacity - total * rb, off, NULL, &n);
+        if (st != VX_OK) return st;
+        if (off && total)                                  // the pass wrote offsets relative to its own first record
+            for (uint64_t b = 0; b <= p->g.NBp; b++) off[b] += total;
+        uint64_t t1 = 0;
+        cudaError_t e = cudaMemcpy(&t1, p->ws + p->g.off_part_base + p->g.P * 8, 8, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(part_base)");
+        t1_total += t1;
+        total += n;
+        if (records_bytes) *records_bytes = (size_t)total * rb;
+    }
+    if (t1_records) *t1_records = t1_total;
+    return VX_OK;
 }
 
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,

@@ -227,7 +227,7 @@ cudaError_t vx_egress_run(const VxGeom &g, uint8_t *ws, bool force_exact, int nu
     }
     if (e == cudaSuccess && ring && !*soft_error) {
         // file sink: the CSR offsets follow the records (they are only complete now), same ring
-        if (ring_push(ring, off_dev, (g.NB + 1) * 8, copy, err, errlen)) *soft_error = 3;
+        if (ring_push(ring, off_dev, (g.NBp + 1) * 8, copy, err, errlen)) *soft_error = 3;
         while (!*soft_error && ring->tail < ring->head)
             if (ring_write_oldest(ring, err, errlen)) *soft_error = 3;
     }

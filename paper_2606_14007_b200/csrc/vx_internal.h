@@ -23,7 +23,9 @@
 #define VX_S2B_ITEMS 9
 #define VX_BIG_TILES_FROM_K 32
 #define VX_STAGE_MAX_BYTES ((size_t)64 << 20) // Table-1 export staging (vx_read_tables)
-#define VX_MAX_MEAN_BUCKET_LOG 9 // K - B <= 9  (mean bucket <= 512 records, BASELINE.json K=33)
+#define VX_MAX_MEAN_BUCKET_LOG 9 // K - B - passes_log <= 9: at most 2^33 records resident (BASELINE.json K=33)
+#define VX_MAX_K 36              // wide Table-2 records keep 4 high nonce bits per nonce
+#define VX_MAX_PASSES_LOG 8
 
 struct VxGeom {
     uint32_t K, B, nonce_size;
@@ -37,8 +39,15 @@ struct VxGeom {
     uint32_t subkey_bits; // = 32: hash bits below the bin index that stage 2's fast ranking compares; a test hook
                           // narrows it so that the tie -> exact re-rank path of a tile runs under test
     uint64_t N;    // 2^K
-    uint64_t P;    // 2^pb
+    uint64_t P;    // partitions resident at a time: 2^(pb - passes_log)
     uint64_t NB;   // 2^B
+    // Bucket-range passes: the plot is made in 2^passes_log passes;
+    // pass s hashes ALL 2^K nonces but keeps only the records whose top passes_log hash bits are s,
+    // i.e. the partitions [p_first, p_first + P) and the buckets [b_first, b_first + NBp).  The
+    // workspace holds one pass; partition, tile and offset indices inside the kernels are relative
+    // to the pass (pb stays the global partition-bit count: it is part of the wide key format).
+    uint32_t passes_log, pass;
+    uint64_t p_first, b_first, NBp;
     uint64_t t2_cap; // Table-2 capacity in records
     uint32_t rec1_bytes, rec2_bytes;
     // workspace carve-up (byte offsets, each 256-aligned)
@@ -86,7 +95,8 @@ struct VxCtrl {
 #endif
 
 // returns false if (K, B) is not a supported geometry
-bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles);
+bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles, uint32_t passes_log = 0);
+void vx_geom_select_pass(VxGeom *g, uint32_t pass);
 
 // host fold of the nonce-independent part of round 1 (vx_blake3.cuh)
 void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_size);

@@ -22,9 +22,11 @@
 template <bool NONCE5>
 __global__ void __launch_bounds__(VX_S1_THREADS)
 vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint64_t N, uint32_t pb, uint32_t cap,
-                  uint32_t cap_check, uint4 *__restrict__ part, uint32_t *__restrict__ cursor,
-                  VxCtrl *__restrict__ ctrl)
+                  uint32_t cap_check, uint32_t p_first, uint32_t p_count, uint4 *__restrict__ part,
+                  uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
 {
+    // p_first, p_count: the partitions this pass keeps (all 2^pb of them unless the plot is made in
+    // bucket-range passes); a record of any other partition is hashed and dropped
     // nonces [n_begin, N): the whole plot, or one round of it (wide layout, vx_launch_stage1)
     const uint64_t base = n_begin + (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
     uint64_t H[VX_S1_NPT];
@@ -37,8 +39,9 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint
     for (int k = 0; k < VX_S1_NPT; k++) {
         const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
         if (n < N) {
-            const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
-            VX_CHECK(ctrl, pb == 0 || p < (1u << pb));
+            const uint32_t p = (pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u) - p_first;
+            if (p >= p_count) continue;
+            VX_CHECK(ctrl, pb == 0 || p + p_first < (1u << pb));
             const uint32_t slot = atomicAdd(&cursor[p], 1u);
             if (slot < cap_check) {                     // = cap, unless a test lowered it
                 VX_CHECK(ctrl, slot < cap);
@@ -76,6 +79,8 @@ vx_k_compact(const uint4 *__restrict__ tmp, uint32_t *__restrict__ cursor_tmp, u
     const uint32_t nsub = 1u << d;
     const uint32_t cnt_raw = cursor_tmp[p];
     const uint32_t cnt = min(cnt_raw, cap_tmp);
+    // (p and the final partitions (p << d) + s are indices within the pass; the low d bits of the
+    // global partition index H >> (64 - pb) are those of the local one: a pass starts on a multiple of 2^d)
     if (tid < nsub) { s_base[tid] = cursor[(p << d) + tid]; s_cnt[tid] = 0u; }
     if (tid == 0 && cnt_raw > cap_tmp) atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
     __syncthreads();
@@ -99,7 +104,7 @@ vx_k_compact(const uint4 *__restrict__ tmp, uint32_t *__restrict__ cursor_tmp, u
             VX_CHECK(ctrl, s < nsub && nsub <= VX_CP_MAXSUB);
             if (slot < cap_check) {
                 const size_t at = (size_t)((p << d) + s) * cap + slot;
-                VX_CHECK(ctrl, slot < cap && ((p << d) + s) < (1u << pb));
+                VX_CHECK(ctrl, slot < cap && ((p << d) + s) < gridDim.x << d);
                 part_a[at] = (H << pb) | (n >> nlo_bits);
                 part_b[at] = (uint16_t)(n & ((1u << nlo_bits) - 1u));
             } else {
@@ -240,8 +245,11 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
     // ctrl + cursors (the wide layout's scratch cursors follow the final ones in the workspace plan)
     cudaError_t e = vx_launch_clear(st, ctrl, sizeof(VxCtrl), cursor, g.P * sizeof(uint32_t), nullptr, nullptr);
     if (e != cudaSuccess) return e;
+    const uint32_t d_tmp = g.pb - g.pb_tmp;                          // final partitions per scratch partition, log2
+    const uint32_t P_tmp = (uint32_t)(g.P >> d_tmp);                 // scratch partitions of this pass
+    const uint32_t p_first_tmp = (uint32_t)(g.p_first >> d_tmp);
     if (g.wide) {
-        e = vx_launch_clear(st, ws + g.off_cursor_tmp, sizeof(uint32_t) << g.pb_tmp, nullptr, 0, nullptr, nullptr);
+        e = vx_launch_clear(st, ws + g.off_cursor_tmp, sizeof(uint32_t) * P_tmp, nullptr, 0, nullptr, nullptr);
         if (e != cudaSuccess) return e;
     }
     const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
@@ -258,13 +266,13 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
         for (uint32_t r = 0; r < g.rounds; r++) {
             if (g.nonce_size == 5)
                 vx_k_hash_scatter<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
-                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
+                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, p_first_tmp, P_tmp, tmp, cursor_tmp, ctrl);
             else
                 vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
-                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, tmp, cursor_tmp, ctrl);
+                    hc, r * slice, (r + 1) * slice, g.pb_tmp, g.cap_tmp, g.cap_tmp, p_first_tmp, P_tmp, tmp, cursor_tmp, ctrl);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;
-            vx_k_compact<<<1u << g.pb_tmp, VX_CP_THREADS, 0, st>>>(
+            vx_k_compact<<<P_tmp, VX_CP_THREADS, 0, st>>>(
                 tmp, cursor_tmp, g.cap_tmp, g.pb, g.pb - g.pb_tmp, g.tile_log, g.cap, g.cap_check,
                 (unsigned long long *)part, part_b, cursor, ctrl);
             e = cudaGetLastError();
@@ -272,7 +280,8 @@ cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws
         }
     } else {
         const uint64_t grid = (g.N + per_cta - 1) / per_cta;
-        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, 0ull, g.N, g.pb, g.cap, g.cap_check, part, cursor, ctrl);
+        vx_k_hash_scatter<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, 0ull, g.N, g.pb, g.cap, g.cap_check,
+                                                                           (uint32_t)g.p_first, (uint32_t)g.P, part, cursor, ctrl);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

@@ -44,7 +44,7 @@ struct VxS2Params {
     unsigned long long *t1_off;
     uint2 *t2_rec;               // external Table-2 records (nonce1, nonce2)
     unsigned long long *t2_off;
-    unsigned long long N, NB, t2_cap;
+    unsigned long long N, NB, t2_cap;   // NB: buckets of this pass (all 2^B unless the plot is made in passes)
     uint32_t P, cap, pb, fb, K, B, do_match, force_exact;
     uint32_t submask;            // sub-key bits the fast ranking pass compares (~0; a test hook narrows it)
     // this launch sorts the partitions [tile_begin, tile_end): the whole plot, or one slice of it
@@ -546,8 +546,8 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 template <bool WIDE, int NS>
 __global__ void __launch_bounds__(256)
 vx_k_export_t1(const uint4 *__restrict__ part, const uint16_t *__restrict__ part_b,
-               const unsigned long long *__restrict__ part_base, uint32_t P, uint32_t cap, uint32_t pb,
-               uint32_t nlo_bits,
+               const unsigned long long *__restrict__ part_base, uint32_t P, uint32_t p_first, uint32_t cap,
+               uint32_t pb, uint32_t nlo_bits,
                unsigned long long first, unsigned long long count, uint8_t *__restrict__ out)
 {
     for (unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; r < count;
@@ -563,7 +563,7 @@ vx_k_export_t1(const uint4 *__restrict__ part, const uint16_t *__restrict__ part
         unsigned long long H, n;
         if constexpr (WIDE) {
             const unsigned long long a = reinterpret_cast<const unsigned long long *>(part)[slot];
-            H = pb ? ((unsigned long long)lo << (64 - pb)) | (a >> pb) : a;
+            H = pb ? ((unsigned long long)(lo + p_first) << (64 - pb)) | (a >> pb) : a;   // p_first: first partition of the pass
             n = ((a & ((1ull << pb) - 1ull)) << nlo_bits) | part_b[slot];
         } else {
             const uint4 rec = part[slot];
@@ -613,11 +613,11 @@ cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, ui
     const unsigned long long *pbase = (const unsigned long long *)(ws + g.off_part_base);
     uint8_t *out = ws + g.off_stage;
     if (g.nonce_size == 5)
-        vx_k_export_t1<true, 5><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, g.tile_log, first, count, out);
+        vx_k_export_t1<true, 5><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, (uint32_t)g.p_first, g.cap, g.pb, g.tile_log, first, count, out);
     else if (g.wide)
-        vx_k_export_t1<true, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, g.tile_log, first, count, out);
+        vx_k_export_t1<true, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, (uint32_t)g.p_first, g.cap, g.pb, g.tile_log, first, count, out);
     else
-        vx_k_export_t1<false, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, g.cap, g.pb, g.tile_log, first, count, out);
+        vx_k_export_t1<false, 4><<<(unsigned)grid, 256, 0, st>>>(part, part_b, pbase, (uint32_t)g.P, (uint32_t)g.p_first, g.cap, g.pb, g.tile_log, first, count, out);
     return cudaGetLastError();
 }
 
@@ -678,7 +678,7 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.t1_off = (unsigned long long *)(ws + g.off_t1_off);
     q.t2_rec = (uint2 *)(ws + g.off_t2_rec);
     q.t2_off = (unsigned long long *)(ws + g.off_t2_off);
-    q.N = g.N; q.NB = g.NB; q.t2_cap = g.t2_check;
+    q.N = g.N; q.NB = g.NBp; q.t2_cap = g.t2_check;      // bucket indices in the kernel are relative to the pass
     q.P = (uint32_t)g.P; q.cap = g.cap; q.cap_check = g.cap_check; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;

@@ -28,8 +28,11 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_workspace_bytes_arithmetic():
-    assert vx.workspace_bytes(0) == 0 and vx.workspace_bytes(41) == 0
-    assert vx.workspace_bytes(34) == 0                     # K - B <= 9
+    assert vx.workspace_bytes(0) == 0 and vx.workspace_bytes(41) == 0 and vx.workspace_bytes(37) == 0
+    # K = 34..36: bucket-range passes, each the size of a K = 33 plot
+    assert 170e9 < vx.workspace_bytes(34) < 178e9 and 170e9 < vx.workspace_bytes(36) < 178e9
+    assert vx.workspace_bytes(20, 24, vx.VX_CREATE_PASSES_LOG(2)) < vx.workspace_bytes(20, 24)
+    assert vx.workspace_bytes(12, 24, vx.VX_CREATE_PASSES_LOG(1)) == 0   # one partition cannot be split
     a, b = vx.workspace_bytes(27), vx.workspace_bytes(28)
     assert 0 < a < b
     # K=31: Table 1 in place in the partition array (2^31 x 16 B x 1.125 slack = 38.7 GB)
