@@ -156,6 +156,7 @@ def make_config(K: int):
     return {"workload": f"K={K} plot: 2^{K} nonces, key SplitMix64({vx_inputs.seed_for_K(K)}), 2^24 buckets "
                         f"(BASELINE.json configs[{idx}])",
             "K": K, "bucket_bits": BUCKET_BITS, "plots_per_gpu": 1,
+            "passes": 1 if K <= 33 else 1 << (K - 33),
             "l2": "inputs larger than L2 (tens of GB of tables are rewritten every step)"}
 
 
@@ -297,12 +298,17 @@ def run_cuda(args):
     N = 1 << K
     stream = torch.cuda.current_stream()
 
+    passes = plot.passes          # > 1 from K = 34: bucket-range passes, each hashing all nonces
+
     def step(evs=None):
-        if evs: evs[0].record(stream)
-        plot.build_table1(stream)
-        if evs: evs[1].record(stream)
-        plot.sort_match_table2(stream)
-        if evs: evs[2].record(stream)
+        for s in range(passes):
+            if passes > 1:
+                plot.select_pass(s)
+            if evs: evs[3 * s].record(stream)
+            plot.build_table1(stream)
+            if evs: evs[3 * s + 1].record(stream)
+            plot.sort_match_table2(stream)
+            if evs: evs[3 * s + 2].record(stream)
 
     for _ in range(args.warmup):
         step()
@@ -310,7 +316,7 @@ def run_cuda(args):
     stats = plot.get_stats()
 
     # ---- device-timed region -------------------------------------------------------------
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3 * passes)] for _ in range(args.steps)]
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -331,9 +337,9 @@ def run_cuda(args):
         clocks["sampled_during"] = ("the timed region" if extra == 0 else
                                     f"the timed region + {extra} untimed steps of the same workload right behind it")
     barrier()
-    total_ms = evs[0][0].elapsed_time(evs[-1][2])
-    s1_ms = [e[0].elapsed_time(e[1]) for e in evs]
-    s2_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    total_ms = evs[0][0].elapsed_time(evs[-1][-1])
+    s1_ms = [sum(e[3 * s].elapsed_time(e[3 * s + 1]) for s in range(passes)) for e in evs]
+    s2_ms = [sum(e[3 * s + 1].elapsed_time(e[3 * s + 2]) for s in range(passes)) for e in evs]
     plot.synchronize()
 
     # ---- end to end through the C ABI with host buffers -----------------------------------
@@ -342,7 +348,28 @@ def run_cuda(args):
     e2e_steps = max(1, args.e2e_steps if args.e2e_steps > 0 else args.steps)
     d2h = 0
     streamed = not args.e2e_serial
-    if streamed:
+    if passes > 1:
+        # K >= 34: the whole Table 2 (172 GB at K = 34) does not fit this box's host memory, so every pass
+        # streams its slice through a pinned ring of 4 MB chunks to a file descriptor (/dev/null here)
+        streamed = False
+        ring = torch.empty(256 << 20, dtype=torch.uint8, pin_memory=True)
+        copy_stream = torch.cuda.Stream()
+        devnull = os.open("/dev/null", os.O_WRONLY)
+        e2e_what = (f"vx_plot_create(key) + per pass ({passes}): vx_build_table1 + vx_sort_match_table2_to_file(Table 2 + "
+                    f"offsets through a 256 MB pinned ring of 4 MB chunks to /dev/null, {args.e2e_slices} slices)")
+
+        def e2e_step():
+            nonlocal d2h
+            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace, flags=args.flags)
+            moved = 0
+            for s in range(passes):
+                p2.select_pass(s)
+                p2.build_table1(stream)
+                moved += p2.sort_match_table2_to_file(copy_stream, devnull, ring.data_ptr(), ring.numel(),
+                                                      slices=args.e2e_slices, stream=stream)
+            d2h = moved
+            p2.free()
+    elif streamed:
         # vx_sort_match_table2_to_host: stage 2 in slices, each finished slice copied
         # on a second stream straight into place in one pinned buffer while later slices are matched
         rec_cap = plot.rec2_bytes * plot.t2_capacity
@@ -355,7 +382,9 @@ def run_cuda(args):
             pinned_rec = torch.empty(rec_cap, dtype=torch.uint8, pin_memory=True)
         except (RuntimeError, ImportError):
             streamed = False                         # not enough pinnable host memory: ranged reads
-    if streamed:
+    if passes > 1:
+        pass
+    elif streamed:
         copy_stream = torch.cuda.Stream()
         pinned_off = torch.empty(nb + 1, dtype=torch.int64, pin_memory=True)
         e2e_what = ("vx_plot_create(key) + vx_build_table1 + vx_sort_match_table2_to_host(Table 2 + offsets into "
@@ -459,7 +488,7 @@ def run_cuda(args):
                     "d2h_bytes_per_step": d2h, "seconds_per_step": e2e_s, "steps": e2e_steps,
                     "seconds_each_rank0": [round(x, 4) for x in e2e_each],
                     "what": e2e_what, "two_plots_in_flight": farm},
-            "gpu_launches": plot.launches_per_plot * args.steps,
+            "gpu_launches": plot.launches_per_plot * passes * args.steps,
             "clocks": clocks,
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -128,7 +128,8 @@ vx_status vx_sort_match_table2(vx_plot *p, void *cuda_stream);
  * _to_file: the same stream of bytes goes to file descriptor fd with sequential write()s of 4 MB
  *   through pinned_staging (HOST, pinned, caller-owned, >= 8 MB; used as a ring of 4 MB chunks, up
  *   to 1024 of them): records, then the (2^B + 1) uint64 offsets, then a 32-byte trailer
- *   {"VXT2\0\0\0\1", u32 K, u32 B, u32 NONCE_SIZE, u32 0, u64 |Table 2|}.  The paper's plot-file
+ *   {"VXT2\0\0\0\1", u32 K, u32 B, u32 NONCE_SIZE, u32 pass | log2(passes) << 16, u64 |Table 2|}
+ *   (a plot made in passes, below: the records and the 2^B / passes + 1 offsets of the selected pass).  The paper's plot-file
  *   format is unpublished; this layout is this library's own.  *file_bytes = bytes
  *   written.  VX_ERR_IO if a write fails. */
 vx_status vx_sort_match_table2_to_host(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,

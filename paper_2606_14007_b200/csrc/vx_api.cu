@@ -443,8 +443,6 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
 {
     if (!p) return VX_ERR_ARG;
     if (fd < 0 || !pinned_staging) return fail(p, VX_ERR_ARG, "bad file descriptor or NULL staging buffer");
-    if (p->g.passes_log)
-        return fail(p, VX_ERR_UNSUPPORTED, "the file sink writes one pass; a plot made in passes goes through vx_plot_all_passes_to_host");
     VxRing *ring = vx_ring_create(pinned_staging, staging_bytes, fd);
     if (!ring) return fail(p, VX_ERR_ARG, "staging buffer smaller than two 4 MB chunks");
     uint64_t n = 0;
@@ -454,7 +452,8 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
     if (s == VX_OK) {
         // trailer: magic, K, B, NONCE_SIZE, reserved, |Table 2|  (all little-endian)
         uint8_t tr[32] = {'V', 'X', 'T', '2', 0, 0, 0, 1};
-        const uint32_t w[4] = {p->g.K, p->g.B, p->g.nonce_size, 0u};
+        // (a plot made in passes: this file is the selected pass's slice; the last word says which of how many)
+        const uint32_t w[4] = {p->g.K, p->g.B, p->g.nonce_size, p->g.pass | (p->g.passes_log << 16)};
         memcpy(tr + 8, w, 16);
         memcpy(tr + 24, &n, 8);
         char msg[128];

@@ -82,7 +82,7 @@ def device_views(plot):
     import torch
     t1, t1o, t2, t2o, pbase = plot.device_tables()
     ws, base = plot.workspace, plot.workspace.data_ptr()
-    P, cap, NB = 1 << plot.partition_bits, plot.partition_capacity, 1 << plot.bucket_bits
+    P, cap, NB = (1 << plot.partition_bits) // plot.passes, plot.partition_capacity, (1 << plot.bucket_bits) // plot.passes
     part = ws[t1 - base: t1 - base + P * cap * 16].view(torch.int32).view(P, cap, 4)
     pb = ws[pbase - base: pbase - base + (P + 1) * 8].view(torch.int64)
     o1 = ws[t1o - base: t1o - base + (NB + 1) * 8].view(torch.int64)
@@ -169,7 +169,8 @@ def sorted_runs(plot, chunk_records=1 << 24):
     rebuilt from the partition index and a = (H << pb) | (n >> t), the nonce from a and b (include/vx.h)."""
     import torch
     pbits, cap, t = plot.partition_bits, plot.partition_capacity, plot.tile_log
-    P = 1 << pbits
+    P = (1 << pbits) // plot.passes                      # resident partitions (one pass)
+    p_first = getattr(plot, "pass_index", 0) * P
     dev = plot.device
     lane = torch.arange(cap, device=dev)[None, :]
     step = max(1, chunk_records // cap)
@@ -184,7 +185,7 @@ def sorted_runs(plot, chunk_records=1 << 24):
         if plot.wide:
             ak = a[p0:p1][valid]
             bk = (b[p0:p1].long() & 0xffff)[valid]
-            pid = torch.arange(p0, p1, device=dev)[:, None].expand(p1 - p0, cap)[valid]
+            pid = torch.arange(p_first + p0, p_first + p1, device=dev)[:, None].expand(p1 - p0, cap)[valid]
             H = t_lsr(ak, pbits) if pbits else ak
             if pbits:
                 H = H | (pid << (64 - pbits))
@@ -232,10 +233,14 @@ def whole_table2_digest_check(plot, K):
     assert total == M, (total, M)
     t1, t1o, t2, t2o, pbase = plot.device_tables()
     base = plot.workspace.data_ptr()
-    o2 = plot.workspace[t2o - base: t2o - base + (NB + 1) * 8].view(torch.int64)
+    b_lo, b_hi = plot.pass_buckets()                      # all 2^B buckets unless the plot is made in passes
+    NBp = b_hi - b_lo
+    o2 = plot.workspace[t2o - base: t2o - base + (NBp + 1) * 8].view(torch.int64)
+    assert int(want_c[:b_lo].sum()) == 0 and int(want_c[b_hi:].sum()) == 0
+    want_c, want_D = want_c[b_lo:b_hi], want_D[b_lo:b_hi]
     assert bool((o2[1:] - o2[:-1] == want_c).all()), "a bucket's Table-2 count differs from the exact match count"
-    got_c = torch.zeros(NB, dtype=torch.int64, device=dev)
-    got_D = torch.zeros(NB, dtype=torch.int64, device=dev)
+    got_c = torch.zeros(NBp, dtype=torch.int64, device=dev)
+    got_D = torch.zeros(NBp, dtype=torch.int64, device=dev)
     step = 1 << 25
     for r0 in range(0, M, step):
         r1 = min(M, r0 + step)
@@ -372,7 +377,8 @@ def wide_views(plot):
     import torch
     t1, t1o, t2, t2o, pbase = plot.device_tables()
     ws, base = plot.workspace, plot.workspace.data_ptr()
-    P, cap, NB = 1 << plot.partition_bits, plot.partition_capacity, 1 << plot.bucket_bits
+    # (a plot made in passes keeps one pass resident: its partitions and its buckets)
+    P, cap, NB = (1 << plot.partition_bits) // plot.passes, plot.partition_capacity, (1 << plot.bucket_bits) // plot.passes
     a_off = t1 - base
     b_off = (a_off + P * cap * 8 + 255) & ~255
     a = ws[a_off: a_off + P * cap * 8].view(torch.int64).view(P, cap)
@@ -383,40 +389,32 @@ def wide_views(plot):
     return a, b, pb, o1, o2
 
 
-def test_K33_full_size_samples_and_properties(vx):
-    """BASELINE.json configs[4]: 2^33 nonces, 5-byte nonces, ~512 records per bucket, 174 GB of
-    tables on one B200.  Sampled buckets hash by hash against the oracle (5-byte keyed hash) with
-    their Table 2 bit-exact; whole-table properties on the device: every nonce exactly once, every
-    partition sorted by (H, n), every stored hash equal to the hash stream (recomputed range by range,
-    itself spot-checked against the oracle), CSR offsets consistent, and EVERY bucket of Table 2 equal in
-    count and content digest to the exact match set of the sorted Table 1."""
+def check_wide_pass(plot, K, key, n_seen, sample_starts, sample_width, R=None):
+    """One resident pass of a plot in the wide layout (K = 33: the whole plot; K = 34: one of two
+    bucket-range passes).  Sampled buckets hash by hash against the oracle with their Table 2 bit-exact;
+    on the device over the whole pass: every partition sorted by (H, n), every stored hash equal to the
+    hash stream (recomputed range by range, itself spot-checked against the oracle), no nonce twice,
+    CSR offsets consistent, and EVERY bucket of Table 2 equal in count and content digest to the exact
+    match set of the sorted Table 1.  n_seen[r] accumulates the nonces of range r met (over the passes)."""
     import torch
-    K, B = 33, 24
-    torch.cuda.empty_cache()
-    free, total = torch.cuda.mem_get_info()
-    need = vx.workspace_bytes(K)
-    if free < need + (6 << 30):
-        pytest.skip(f"needs {need / 1e9:.0f} GB + 6 GB of device memory, {free / 1e9:.0f} GB free")
-    key = vx_inputs.config_key(K)
-    plot = vx.Plot(K, key, B)
-    assert plot.nonce_size == 5
-    plot.build_table1()
-    plot.sort_match_table2()
-    stats = plot.get_stats()
+    B = plot.bucket_bits
     N = 1 << K
-    assert stats["t1_records"] == N
-    rng = np.random.default_rng(33)
-    starts = [0, (1 << 24) - 4] + [int(x) for x in rng.integers(0, (1 << 24) - 4, 14)]
-    n = check_sampled_buckets(plot, K, key, [(s, s + 4) for s in starts])
+    stats = plot.get_stats()
+    b_lo, b_hi = plot.pass_buckets()
+    n = check_sampled_buckets(plot, K, key, [(b_lo + s, b_lo + s + sample_width) for s in sample_starts])
     assert n > 25000
-
     a, b, pb, o1, o2 = wide_views(plot)
+    NBp = b_hi - b_lo
+    o1, o2 = o1[:NBp + 1], o2[:NBp + 1]
     dev = plot.device
     pbits, cap = plot.partition_bits, plot.partition_capacity
-    P = 1 << pbits
+    P = (1 << pbits) // plot.passes
+    p_first = plot.pass_index * P
+    a, b, pb = a[:P], b[:P], pb[:P + 1]
     cnt = pb[1:] - pb[:-1]
-    assert int(pb[0]) == 0 and int(pb[-1]) == N and int(cnt.max()) <= cap
-    assert int(o1[0]) == 0 and int(o1[-1]) == N and bool((o1[1:] >= o1[:-1]).all())
+    Np = stats["t1_records"]
+    assert int(pb[0]) == 0 and int(pb[-1]) == Np and int(cnt.max()) <= cap
+    assert int(o1[0]) == 0 and int(o1[-1]) == Np and bool((o1[1:] >= o1[:-1]).all())
     assert stats["max_bucket"] == int((o1[1:] - o1[:-1]).max())
     assert int(o2[0]) == 0 and int(o2[-1]) == stats["t2_records"] and bool((o2[1:] >= o2[:-1]).all())
     # bucket b of partition q starts at slot offsets[b] - part_base[q]: bucket sizes sum to the partition
@@ -425,18 +423,20 @@ def test_K33_full_size_samples_and_properties(vx):
     lane = torch.arange(cap, device=dev)[None, :]
     chunk = (1 << 25) // cap
     lowmask = (1 << pbits) - 1
-    # per pass over Table 1: a nonce range of R nonces, its hash stream recomputed by vx_hash_range
-    # (the 68 GB stream of all 2^33 hashes does not fit beside the tables)
-    free, _ = torch.cuda.mem_get_info()
-    R = 1 << 30 if free > (14 << 30) else 1 << 29 if free > (8 << 30) else 1 << 28
-    rng = np.random.default_rng(33)
-    for r0 in range(0, N, R):
+    # per sweep over Table 1: a nonce range of R nonces, its hash stream recomputed by vx_hash_range
+    # (the stream of all 2^K hashes does not fit beside the tables)
+    if R is None:
+        free, _ = torch.cuda.mem_get_info()
+        R = 1 << 30 if free > (14 << 30) else 1 << 29 if free > (8 << 30) else 1 << 28
+    rng = np.random.default_rng(K)
+    for ri, r0 in enumerate(range(0, N, R)):
         seen = torch.zeros(R, dtype=torch.bool, device=dev)
         hashes = plot.hash_range(r0, R)
-        pick = np.unique(rng.integers(0, R, 1 << 13))     # the stream against the oracle, 5-byte nonces
+        pick = np.unique(rng.integers(0, R, 1 << 12))     # the stream against the oracle, 5-byte nonces
         got = hashes[torch.from_numpy(pick).to(dev)].cpu().numpy().view(np.uint64)
         want = np.array([oracle.hash_nonce(key, int(r0 + n), 5) for n in pick], dtype=np.uint64)
         assert np.array_equal(got, want), "the hash stream differs from the oracle"
+        met = 0
         for p0 in range(0, P, chunk):
             ak = a[p0:p0 + chunk]
             valid = lane < cnt[p0:p0 + chunk, None]
@@ -451,15 +451,75 @@ def test_K33_full_size_samples_and_properties(vx):
             sel = valid & (non >= r0) & (non < r0 + R)
             idx = non[sel] - r0
             seen[idx] = True
+            met += int(sel.sum())
             # the stored hash (partition index = its top pb bits, a >> pb = the rest) is the nonce's hash
-            pid = torch.arange(p0, p0 + ak.shape[0], device=dev)[:, None].expand_as(ak)
+            pid = torch.arange(p_first + p0, p_first + p0 + ak.shape[0], device=dev)[:, None].expand_as(ak)
             Hrec = (pid[sel] << (64 - pbits)) | t_lsr(ak[sel], pbits)
             assert bool((hashes[idx] == Hrec).all()), "a stored hash differs from the hash stream"
             del ak, valid, bk, non, sel, idx, pid, Hrec
-        assert int(seen.sum()) == R, "some nonce is missing from Table 1 (or appears twice)"
+        assert int(seen.sum()) == met, "a nonce appears twice in Table 1"
+        n_seen[ri] = n_seen.get(ri, 0) + met
         del seen, hashes
     # Table 2, every bucket: count and content digest against the exact match set of the sorted Table 1
     whole_table2_digest_check(plot, K)
+    return R, stats
+
+
+def test_K33_full_size_samples_and_properties(vx):
+    """BASELINE.json configs[4]: 2^33 nonces, 5-byte nonces, ~512 records per bucket, 174 GB of
+    tables on one B200 (check_wide_pass)."""
+    import torch
+    K, B = 33, 24
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    need = vx.workspace_bytes(K)
+    if free < need + (6 << 30):
+        pytest.skip(f"needs {need / 1e9:.0f} GB + 6 GB of device memory, {free / 1e9:.0f} GB free")
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    assert plot.nonce_size == 5 and plot.passes == 1
+    plot.pass_index = 0
+    plot.build_table1()
+    plot.sort_match_table2()
+    rng = np.random.default_rng(33)
+    starts = [0, (1 << 24) - 4] + [int(x) for x in rng.integers(0, (1 << 24) - 4, 14)]
+    n_seen = {}
+    R, stats = check_wide_pass(plot, K, key, n_seen, starts, 4)
+    assert stats["t1_records"] == 1 << K
+    assert all(v == R for v in n_seen.values()) and len(n_seen) == (1 << K) // R   # every nonce exactly once
+    plot.free()
+
+
+def test_K34_two_bucket_range_passes(vx):
+    """K = 34: 2^34 nonces in two bucket-range passes, each the size of
+    a K = 33 plot and checked like one; over the two passes every nonce is met exactly once."""
+    import torch
+    K, B = 34, 24
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    need = vx.workspace_bytes(K)
+    if free < need + (6 << 30):
+        pytest.skip(f"needs {need / 1e9:.0f} GB + 6 GB of device memory, {free / 1e9:.0f} GB free")
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    assert plot.nonce_size == 5 and plot.passes == 2
+    n_seen = {}
+    t1 = t2 = 0
+    for s in range(plot.passes):
+        plot.select_pass(s)
+        plot.pass_index = s
+        plot.build_table1()
+        plot.sort_match_table2()
+        NBp = (1 << B) // plot.passes
+        rng = np.random.default_rng(34 + s)
+        starts = [0, NBp - 2] + [int(x) for x in rng.integers(0, NBp - 2, 12)]
+        R, stats = check_wide_pass(plot, K, key, n_seen, starts, 2, R=1 << 28)   # the same ranges in both passes
+        t1 += stats["t1_records"]
+        t2 += stats["t2_records"]
+    assert t1 == 1 << K
+    assert all(v == R for v in n_seen.values()) and len(n_seen) == (1 << K) // R   # every nonce exactly once
+    mean = (1 << K) * (1 - 2.0 ** (B - K - 1))
+    assert abs(t2 - mean) < 8 * mean ** 0.5
     plot.free()
 
 

@@ -110,16 +110,26 @@ def test_pass_arguments(vx):
     with pytest.raises(vx.VxError) as ei:
         plot.select_pass(4)
     assert ei.value.status == -1
-    # the file sink is one pass only
+    # the file sink writes the selected pass's slice: records, its 2^B / passes + 1 offsets, trailer
     import os
+    import tempfile
     import torch
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(18, key, 12)
     ring = torch.empty(16 << 20, dtype=torch.uint8, pin_memory=True)
-    fd = os.open("/dev/null", os.O_WRONLY)
-    try:
+    plot.select_pass(2)
+    b0, b1 = plot.pass_buckets()
+    with tempfile.TemporaryFile() as f:
         plot.build_table1()
-        with pytest.raises(vx.VxError) as ei:
-            plot.sort_match_table2_to_file(torch.cuda.Stream(), fd, ring.data_ptr(), ring.numel())
-        assert ei.value.status == -7
-    finally:
-        os.close(fd)
+        n = plot.sort_match_table2_to_file(torch.cuda.Stream(), f.fileno(), ring.data_ptr(), ring.numel(), slices=3)
+        f.seek(0)
+        blob = np.frombuffer(f.read(), dtype=np.uint8)
+    m = int(o_t2o[b1] - o_t2o[b0])
+    assert n == len(blob) == 8 * m + 8 * (b1 - b0 + 1) + 32
+    offs = blob[8 * m: 8 * m + 8 * (b1 - b0 + 1)].view(np.uint64)
+    assert np.array_equal(offs, o_t2o[b0:b1 + 1] - o_t2o[b0])
+    g1, g2 = canon_t2(offs, *decode_t2(blob[:8 * m], 4))
+    assert np.array_equal(g1, o_n1[int(o_t2o[b0]):int(o_t2o[b1])]) and np.array_equal(g2, o_n2[int(o_t2o[b0]):int(o_t2o[b1])])
+    tr = blob[-32:]
+    assert bytes(tr[:8]) == b"VXT2\0\0\0\1"
+    assert list(tr[8:24].view(np.uint32)) == [18, 12, 4, 2 | (2 << 16)] and int(tr[24:].view(np.uint64)[0]) == m
     plot.free()
