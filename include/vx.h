@@ -162,6 +162,31 @@ vx_status vx_plot_all_passes_to_host(vx_plot *p, void *compute_stream, void *cop
                                      void *host_records, size_t records_capacity, uint64_t *host_offsets,
                                      size_t *records_bytes, uint64_t *t1_records);
 
+/* One plot over G = 2, 4 or 8 GPUs (the paper's machines hold 8
+ * GPUs each and use one).  Rank r hashes the nonces [r 2^K / G, (r + 1) 2^K / G); buckets are owned by
+ * hash range, rank g owning the buckets [g 2^B / G, (g + 1) 2^B / G) (vx_shard_owner: host arithmetic
+ * only).  The exchange is fused with the first partition pass: the hashing thread claims a slot with an
+ * atomic on the OWNER's partition cursor and stores the 16-byte record into the OWNER's partition array
+ * through peer pointers (NVLink / NVSwitch peer access, or one device in tests) -- one all-to-all,
+ * nothing staged.  After it every rank holds exactly slice r of the plot and runs
+ * vx_sort_match_table2* / vx_read_tables on it as on a selected pass (no further communication).
+ *   Each rank: vx_plot_create_opts(K, key, B, VX_CREATE_PASSES_LOG(log2 G)) with the SAME key, bind a
+ *   workspace, then
+ *     vx_shard_begin(p, r, G, stream)            zero this rank's cursors             -- BARRIER over all ranks
+ *     vx_shard_scatter(p, r, G, peers, stream)   hash the share, store at the owners  -- BARRIER over all ranks
+ *     vx_shard_finish(p, stream)                 scan this rank's partitions; Table 1 slice built
+ *   dev_peer_workspaces[g] (HOST array of G DEVICE pointers valid on this device: the bound workspace
+ *   of rank g's plot, e.g. mapped with cudaIpcOpenMemHandle; entry r is this plot's own).  The barriers
+ *   (stream-complete on every rank, e.g. torch.distributed.barrier after a stream synchronize) are the
+ *   caller's.  16-byte record layout only (K <= 32): VX_ERR_UNSUPPORTED in the wide layout.
+ *   Measured on one device only (two workspaces standing for two peers); DESIGN.md says so. */
+vx_status vx_shard_owner(uint32_t K, uint32_t bucket_bits, uint32_t world, uint32_t rank, uint64_t *nonce_begin,
+                         uint64_t *nonce_end, uint64_t *bucket_begin, uint64_t *bucket_end);
+vx_status vx_shard_begin(vx_plot *p, uint32_t rank, uint32_t world, void *cuda_stream);
+vx_status vx_shard_scatter(vx_plot *p, uint32_t rank, uint32_t world, void *const *dev_peer_workspaces,
+                           void *cuda_stream);
+vx_status vx_shard_finish(vx_plot *p, void *cuda_stream);
+
 /* Copy the buckets [bucket_begin, bucket_end) of table 1 or 2 to HOST memory in the external
  * format.  Synchronises the plot's stream.  offsets_out (may be NULL) receives
  * bucket_end - bucket_begin + 1 entries relative to the first record of bucket_begin.

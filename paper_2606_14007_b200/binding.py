@@ -33,7 +33,7 @@ EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_op
            "vx_plot_create_ex", "vx_plot_create_opts",
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
            "vx_sort_match_table2_to_file", "vx_read_tables", "vx_plot_passes", "vx_plot_select_pass",
-           "vx_plot_all_passes_to_host",
+           "vx_plot_all_passes_to_host", "vx_shard_owner", "vx_shard_begin", "vx_shard_scatter", "vx_shard_finish",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink", "vx_probe_alu",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
@@ -100,6 +100,14 @@ def load_library() -> ctypes.CDLL:
     L.vx_plot_all_passes_to_host.restype = ctypes.c_int
     L.vx_plot_all_passes_to_host.argtypes = [_vp, _vp, _vp, _u32, _vp, _sz, _vp, ctypes.POINTER(_sz),
                                              ctypes.POINTER(_u64)]
+    L.vx_shard_owner.restype = ctypes.c_int
+    L.vx_shard_owner.argtypes = [_u32, _u32, _u32, _u32] + [ctypes.POINTER(_u64)] * 4
+    L.vx_shard_begin.restype = ctypes.c_int
+    L.vx_shard_begin.argtypes = [_vp, _u32, _u32, _vp]
+    L.vx_shard_scatter.restype = ctypes.c_int
+    L.vx_shard_scatter.argtypes = [_vp, _u32, _u32, ctypes.POINTER(_vp), _vp]
+    L.vx_shard_finish.restype = ctypes.c_int
+    L.vx_shard_finish.argtypes = [_vp, _vp]
     L.vx_read_tables.restype = ctypes.c_int
     L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
     L.vx_device_tables.restype = ctypes.c_int
@@ -270,6 +278,20 @@ class Plot:
                 offsets_ptr or None, ctypes.byref(need), ctypes.byref(t1)))
         return need.value, t1.value
 
+    # -- one plot over G GPUs (8(f4)) ------------------------------------------------------------
+    def shard_begin(self, rank: int, world: int, stream=None):
+        with self._dev():
+            self._check(self._L.vx_shard_begin(self._h, rank, world, self._sp(stream)))
+
+    def shard_scatter(self, rank: int, world: int, peer_ptrs, stream=None):
+        arr = (_vp * world)(*[int(x) for x in peer_ptrs])
+        with self._dev():
+            self._check(self._L.vx_shard_scatter(self._h, rank, world, arr, self._sp(stream)))
+
+    def shard_finish(self, stream=None):
+        with self._dev():
+            self._check(self._L.vx_shard_finish(self._h, self._sp(stream)))
+
     def synchronize(self):
         with self._dev():
             self._check(self._L.vx_synchronize(self._h))
@@ -350,6 +372,15 @@ def probe_alu(kind: str, iters: int, scratch, ctas_per_sm: int = 8, stream=None)
     if st != VX_OK:
         raise VxError(st, f"vx_probe_alu({kind})")
     return ops.value
+
+
+def shard_owner(K: int, bucket_bits: int, world: int, rank: int):
+    """(nonce_begin, nonce_end, bucket_begin, bucket_end) of a rank of a plot sharded over `world` GPUs."""
+    v = [_u64() for _ in range(4)]
+    st = load_library().vx_shard_owner(K, bucket_bits, world, rank, *[ctypes.byref(x) for x in v])
+    if st != VX_OK:
+        raise VxError(st, f"vx_shard_owner(K={K}, B={bucket_bits}, world={world}, rank={rank})")
+    return tuple(x.value for x in v)
 
 
 def hash_range(K: int, key: bytes, nonce_begin: int, count: int):

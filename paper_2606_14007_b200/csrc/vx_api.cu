@@ -522,6 +522,76 @@ vx_status vx_plot_all_passes_to_host(vx_plot *p, void *compute_stream, void *cop
     return VX_OK;
 }
 
+// ------------------------------------------------------------------------------ one plot over G GPUs (8(f4))
+vx_status vx_shard_owner(uint32_t K, uint32_t bucket_bits, uint32_t world, uint32_t rank, uint64_t *nonce_begin,
+                         uint64_t *nonce_end, uint64_t *bucket_begin, uint64_t *bucket_end)
+{
+    if (K < 1 || K > VX_MAX_K || bucket_bits < 1 || bucket_bits > 24) return VX_ERR_ARG;
+    if (world < 1 || world > VX_MAX_SHARD_WORLD || (world & (world - 1)) || rank >= world) return VX_ERR_ARG;
+    uint32_t wl = 0;
+    while ((1u << wl) < world) wl++;
+    if (wl > K || wl > bucket_bits) return VX_ERR_ARG;
+    if (nonce_begin) *nonce_begin = ((uint64_t)rank << K) >> wl;
+    if (nonce_end) *nonce_end = ((uint64_t)(rank + 1) << K) >> wl;
+    if (bucket_begin) *bucket_begin = ((uint64_t)rank << bucket_bits) >> wl;
+    if (bucket_end) *bucket_end = ((uint64_t)(rank + 1) << bucket_bits) >> wl;
+    return VX_OK;
+}
+
+static vx_status shard_check(vx_plot *p, uint32_t rank, uint32_t world)
+{
+    if (p->state < VX_BOUND) return fail(p, VX_ERR_STATE, "sharded build before vx_plot_bind");
+    if (world != (1u << p->g.passes_log) || world < 2)
+        return fail(p, VX_ERR_ARG, "world must equal the plot's pass count (create with VX_CREATE_PASSES_LOG(log2 world))");
+    if (rank >= world) return fail(p, VX_ERR_ARG, "rank outside [0, world)");
+    if (p->g.wide) return fail(p, VX_ERR_UNSUPPORTED, "the sharded build is implemented for the 16-byte record layout (K <= 32)");
+    return VX_OK;
+}
+
+vx_status vx_shard_begin(vx_plot *p, uint32_t rank, uint32_t world, void *cuda_stream)
+{
+    if (!p) return VX_ERR_ARG;
+    vx_status s = shard_check(p, rank, world);
+    if (s != VX_OK) return s;
+    if (p->state >= VX_BUILT && (s = sync_and_check(p)) != VX_OK && s != VX_ERR_OVERFLOW) return s;
+    vx_geom_select_pass(&p->g, rank);                      // the rank owns slice `rank` of the buckets
+    p->state = VX_BOUND;
+    p->t1_materialised = false;
+    p->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = vx_launch_shard_clear(p->g, p->ws, p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "shard clear launch");
+    return VX_OK;
+}
+
+vx_status vx_shard_scatter(vx_plot *p, uint32_t rank, uint32_t world, void *const *dev_peer_workspaces,
+                           void *cuda_stream)
+{
+    if (!p || !dev_peer_workspaces) return VX_ERR_ARG;
+    vx_status s = shard_check(p, rank, world);
+    if (s != VX_OK) return s;
+    if (p->g.pass != rank) return fail(p, VX_ERR_STATE, "vx_shard_scatter before vx_shard_begin for this rank");
+    for (uint32_t i = 0; i < world; i++)
+        if (!dev_peer_workspaces[i] || ((uintptr_t)dev_peer_workspaces[i] & 255))
+            return fail(p, VX_ERR_ARG, "NULL or misaligned peer workspace");
+    if (dev_peer_workspaces[rank] != p->ws) return fail(p, VX_ERR_ARG, "peer_workspaces[rank] is not this plot's workspace");
+    p->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = vx_launch_shard_scatter(p->g, p->hc, rank, p->g.passes_log, (uint8_t *const *)dev_peer_workspaces, p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "shard scatter launch");
+    return VX_OK;
+}
+
+vx_status vx_shard_finish(vx_plot *p, void *cuda_stream)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_BOUND || !p->g.passes_log) return fail(p, VX_ERR_STATE, "vx_shard_finish before vx_shard_begin");
+    p->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = vx_launch_shard_scan(p->g, p->ws, p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "shard scan launch");
+    p->state = VX_BUILT;
+    p->t1_materialised = false;
+    return VX_OK;
+}
+
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,
                            const void **dev_t2_records, const uint64_t **dev_t2_offsets,
                            const uint64_t **dev_partition_base)

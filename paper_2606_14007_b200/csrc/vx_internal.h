@@ -104,6 +104,15 @@ void vx_hash_const_init(VxHashConst *hc, const uint8_t key[32], uint32_t nonce_s
 // ---------------------------------------------------------------------------------- launches
 cudaError_t vx_launch_stage1(const VxGeom &g, const VxHashConst &hc, uint8_t *ws, cudaStream_t st);
 uint32_t vx_stage1_launches(const VxGeom &g);   // kernels vx_launch_stage1 enqueues
+// one plot over G = 2^world_log GPUs (8(f4)): clear the rank's cursors; hash the rank's nonce share and
+// scatter every record into its owner's workspace (peer_ws[g] = base of rank g's workspace, device
+// pointers valid on this device); scan the rank's own partitions.  The caller puts a barrier over all
+// ranks between the three.
+#define VX_MAX_SHARD_WORLD 8
+cudaError_t vx_launch_shard_clear(const VxGeom &g, uint8_t *ws, cudaStream_t st);
+cudaError_t vx_launch_shard_scatter(const VxGeom &g, const VxHashConst &hc, uint32_t rank, uint32_t world_log,
+                                    uint8_t *const *peer_ws, cudaStream_t st);
+cudaError_t vx_launch_shard_scan(const VxGeom &g, uint8_t *ws, cudaStream_t st);
 // zero two regions and two words with a kernel (not a memset: see vx_k_clear)
 cudaError_t vx_launch_clear(cudaStream_t st, void *a, size_t bytes_a, void *b, size_t bytes_b, uint32_t *w0, uint32_t *w1);
 // sorts (and matches) the partitions [tile_begin, tile_end) -- (0, P) for the whole plot; slices must

@@ -55,6 +55,47 @@ vx_k_hash_scatter(const __grid_constant__ VxHashConst hc, uint64_t n_begin, uint
     }
 }
 
+// ----------------------------------------------------------------------------- one plot over G GPUs
+// SURVEY.md 8(e) / 8(f4) (the paper's boxes hold 8 GPUs, it uses one): rank r hashes
+// the nonces [r 2^K / G, (r + 1) 2^K / G); buckets are owned by hash range -- rank g owns the
+// partitions (and buckets) whose top log2 G hash bits are g -- and the record goes straight from the
+// hashing thread to its owner: the slot is claimed with an atomic on the OWNER's cursor and the
+// 16-byte record stored into the OWNER's partition array, both through peer pointers (NVLink 5 /
+// NVSwitch peer stores: the all-to-all is fused with the first partition pass, nothing is staged
+// or sent twice).  Every rank's workspace has the same carve-up (one "pass" of a plot created with
+// VX_CREATE_PASSES_LOG(log2 G)), so a peer is addressed by its workspace base alone.
+struct VxPeers { uint8_t *ws[VX_MAX_SHARD_WORLD]; };
+
+__global__ void __launch_bounds__(VX_S1_THREADS)
+vx_k_hash_scatter_sharded(const __grid_constant__ VxHashConst hc, const __grid_constant__ VxPeers peers,
+                          uint64_t n_begin, uint64_t n_end, uint32_t pb, uint32_t own_shift, uint32_t cap,
+                          uint32_t cap_check, size_t off_part, size_t off_cursor, size_t off_ctrl)
+{
+    const uint64_t base = n_begin + (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
+    uint64_t H[VX_S1_NPT];
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
+        H[k] = vx_blake3_h<false>(hc, (uint32_t)n, (uint32_t)(n >> 32));
+    }
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t n = base + (uint64_t)k * VX_S1_THREADS;
+        if (n < n_end) {
+            const uint32_t p = (uint32_t)(H[k] >> (64 - pb));          // global partition (pb >= log2 G >= 1)
+            const uint32_t owner = p >> own_shift;                     // its top log2 G bits
+            const uint32_t pl = p & ((1u << own_shift) - 1u);          // partition index at the owner
+            uint8_t *ws = peers.ws[owner];
+            const uint32_t slot = atomicAdd(reinterpret_cast<uint32_t *>(ws + off_cursor) + pl, 1u);
+            if (slot < cap_check)
+                reinterpret_cast<uint4 *>(ws + off_part)[(uint64_t)pl * cap + slot] =
+                    make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)n, (uint32_t)(n >> 32));
+            else
+                atomicOr(&reinterpret_cast<VxCtrl *>(ws + off_ctrl)->flags, VX_FLAG_PART_OVERFLOW);
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------- wide: compaction
 // Stage 1 in rounds (wide layout, K >= 33).  A 10-byte record written
 // straight from the hash kernel costs two scattered store requests plus the atomic, and scattered
@@ -315,3 +356,33 @@ cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t
         vx_k_hash_sink<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, count, dev_sink);
     return cudaGetLastError();
 }
+
+// ----------------------------------------------------------------------------- one plot over G GPUs: launches
+cudaError_t vx_launch_shard_clear(const VxGeom &g, uint8_t *ws, cudaStream_t st)
+{
+    return vx_launch_clear(st, ws + g.off_ctrl, sizeof(VxCtrl), ws + g.off_cursor, g.P * sizeof(uint32_t), nullptr, nullptr);
+}
+
+cudaError_t vx_launch_shard_scatter(const VxGeom &g, const VxHashConst &hc, uint32_t rank, uint32_t world_log,
+                                    uint8_t *const *peer_ws, cudaStream_t st)
+{
+    if (g.wide || world_log != g.passes_log || world_log == 0 || (1u << world_log) > VX_MAX_SHARD_WORLD)
+        return cudaErrorInvalidValue;
+    VxPeers peers;
+    for (uint32_t i = 0; i < VX_MAX_SHARD_WORLD; i++) peers.ws[i] = i < (1u << world_log) ? peer_ws[i] : nullptr;
+    const uint64_t share = g.N >> world_log, n0 = (uint64_t)rank * share;
+    const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
+    const uint64_t grid = (share + per_cta - 1) / per_cta;
+    vx_k_hash_scatter_sharded<<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc, peers, n0, n0 + share, g.pb,
+                                                                        g.pb - world_log, g.cap, g.cap_check,
+                                                                        g.off_part, g.off_cursor, g.off_ctrl);
+    return cudaGetLastError();
+}
+
+cudaError_t vx_launch_shard_scan(const VxGeom &g, uint8_t *ws, cudaStream_t st)
+{
+    vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>((const uint32_t *)(ws + g.off_cursor), g.cap_check, g.P,
+                                                       (unsigned long long *)(ws + g.off_part_base));
+    return cudaGetLastError();
+}
+
