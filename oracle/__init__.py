@@ -78,6 +78,15 @@ def lib() -> ctypes.CDLL:
         L.vxo_table1_from_records.argtypes = [ctypes.c_int, U64, U64, U64, _p64, _p64, _p64, _p64, _p64]
         L.vxo_table2_digest.restype = U64
         L.vxo_table2_digest.argtypes = [ctypes.c_int, ctypes.c_int, U64, U64, _p64, _p64, _p64, _p64, _p64]
+        L.vxo_hash_pair.restype = U64
+        L.vxo_hash_pair.argtypes = [ctypes.c_char_p, U64, U64, ctypes.c_int]
+        L.vxo_table2_rekey.restype = ctypes.c_int
+        L.vxo_table2_rekey.argtypes = [ctypes.c_int, ctypes.c_char_p, ctypes.c_int, U64, _p64, _p64,
+                                       _p64, _p64, _p64, _p64]
+        L.vxo_plot_file_bytes.restype = U64
+        L.vxo_plot_file_bytes.argtypes = [ctypes.c_int, ctypes.c_int, U64]
+        L.vxo_plot_file.restype = None
+        L.vxo_plot_file.argtypes = [ctypes.c_int, ctypes.c_char_p, ctypes.c_int, U64, _p64, _p64, _p64, _p8]
         L.vxo_table1_digest.restype = ctypes.c_int
         L.vxo_table1_digest.argtypes = [ctypes.c_int, ctypes.c_char_p, ctypes.c_int, _p64, _p64]
         _lib = L
@@ -306,6 +315,36 @@ def serialize_t2(nsize: int, n1, n2) -> np.ndarray:
     n2 = np.ascontiguousarray(n2, dtype=np.uint64)
     out = np.empty(len(n1) * 2 * nsize, dtype=np.uint8)
     lib().vxo_serialize_t2(nsize, len(n1), _ptr(n1), _ptr(n2), _ptr8(out))
+    return out
+
+
+# ------------------------------------------------------------------------------- Step 6
+def hash_pair(key: bytes, n1: int, n2: int, nsize: int) -> int:
+    return int(lib().vxo_hash_pair(key, n1, n2, nsize))
+
+
+def table2_rekey(K: int, key: bytes, bucket_bits: int, n1, n2):
+    """Re-keyed Table 2 (A19, A20): (offsets[2^B+1], n1, n2, H2), buckets sorted by (H2, n1, n2)."""
+    n1 = np.ascontiguousarray(n1, dtype=np.uint64)
+    n2 = np.ascontiguousarray(n2, dtype=np.uint64)
+    cnt = len(n1)
+    offsets = np.empty((1 << bucket_bits) + 1, dtype=np.uint64)
+    o1 = np.empty(max(cnt, 1), dtype=np.uint64)
+    o2 = np.empty(max(cnt, 1), dtype=np.uint64)
+    oh = np.empty(max(cnt, 1), dtype=np.uint64)
+    rc = lib().vxo_table2_rekey(K, key, bucket_bits, cnt, _ptr(n1), _ptr(n2), _ptr(offsets), _ptr(o1), _ptr(o2), _ptr(oh))
+    if rc != 0:
+        raise RuntimeError(f"vxo_table2_rekey failed: {rc}")
+    return offsets, o1[:cnt], o2[:cnt], oh[:cnt]
+
+
+def plot_file(K: int, key: bytes, bucket_bits: int, offsets, n1, n2) -> np.ndarray:
+    """The plot file bytes (A21) of a re-keyed Table 2."""
+    offsets = np.ascontiguousarray(offsets, dtype=np.uint64)
+    n1 = np.ascontiguousarray(n1, dtype=np.uint64)
+    n2 = np.ascontiguousarray(n2, dtype=np.uint64)
+    out = np.empty(int(lib().vxo_plot_file_bytes(K, bucket_bits, len(n1))), dtype=np.uint8)
+    lib().vxo_plot_file(K, key, bucket_bits, len(n1), _ptr(offsets), _ptr(n1), _ptr(n2), _ptr8(out))
     return out
 
 

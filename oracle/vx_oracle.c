@@ -19,6 +19,7 @@
  *   Step 4' the same set by "sort the bucket, scan forward while H_j - H_i < T"
  *                      ("insertion sort by hash value ... then pairwise matching")
  *   Step 5  canonical forms and external record bytes                 (A10, A12, A13)
+ *   Step 6  Table 2 re-keyed by the hash of the pair, and the plot file (A19-A21)
  *
  * Everything is integer arithmetic; results are defined bit-exactly.
  *
@@ -483,6 +484,100 @@ uint64_t vxo_table2_digest(int K, int mode, uint64_t b_begin, uint64_t b_end,
         total += m;
     }
     return total;
+}
+
+/* ------------------------------------------------------------------ Step 6: re-keyed Table 2 */
+/* SURVEY.md 8(f2) (plot files a prover searches): Table 2 comes out of the
+ * match step grouped by the bucket of the TABLE-1 hash, so nothing can look a challenge up in it.
+ * The paper does not say how VaultX keys it (the format is unpublished, L183); readings A19-A21 of
+ * DESIGN.md fix this build's own:
+ *   A19  pair hash  H2(n1, n2) = first 8 bytes, read big-endian, of the BLAKE3 keyed hash (same plot
+ *        key, same mode as Step 2) of the external Table-2 record bytes
+ *        nonce1[NONCE_SIZE] LE || nonce2[NONCE_SIZE] LE   (block_len = 2 NONCE_SIZE);
+ *   A20  the re-keyed table holds the same pairs, grouped into 2^B buckets by H2 >> (64 - B), each
+ *        bucket sorted by (H2, n1, n2); CSR offsets;
+ *   A21  plot file = header || offsets || records (vxo_plot_file below).
+ * Parity with VaultX's own files: UNPINNED (as for Table 2 itself). */
+uint64_t vxo_hash_pair(const uint8_t key[32], uint64_t n1, uint64_t n2, int nonce_size)
+{
+    uint8_t msg[16], hb[8];
+    uint64_t H = 0;
+    int i;
+    for (i = 0; i < nonce_size; i++) msg[i] = (uint8_t)(n1 >> (8 * i));
+    for (i = 0; i < nonce_size; i++) msg[nonce_size + i] = (uint8_t)(n2 >> (8 * i));
+    vxo_blake3_keyed(key, msg, (size_t)(2 * nonce_size), hb, 8);
+    for (i = 0; i < 8; i++) H = (H << 8) | hb[i];
+    return H;
+}
+
+typedef struct { uint64_t H, n1, n2; } rk_t;
+
+static int rk_cmp(const void *pa, const void *pb)
+{ /* A20: (H2, n1, n2) ascending */
+    const rk_t *a = (const rk_t *)pa, *b = (const rk_t *)pb;
+    if (a->H != b->H) return a->H < b->H ? -1 : 1;
+    if (a->n1 != b->n1) return a->n1 < b->n1 ? -1 : 1;
+    if (a->n2 != b->n2) return a->n2 < b->n2 ? -1 : 1;
+    return 0;
+}
+
+/* cnt pairs (n1[i], n2[i]) in any order -> offsets[2^B + 1], and the pairs with their hashes in the
+ * canonical order of A20.  Returns 0, -1 bad args, -2 no memory. */
+int vxo_table2_rekey(int K, const uint8_t key[32], int bucket_bits, uint64_t cnt,
+                     const uint64_t *n1, const uint64_t *n2,
+                     uint64_t *offsets, uint64_t *n1_out, uint64_t *n2_out, uint64_t *h2_out)
+{
+    const uint64_t NB = 1ULL << bucket_bits;
+    const int ns = vxo_nonce_size(K);
+    uint64_t i, b, *fill;
+    rk_t *rec, *tmp;
+    if (K < 1 || K > 40 || bucket_bits < 1 || bucket_bits > 32) return -1;
+    rec = (rk_t *)malloc((size_t)(cnt ? cnt : 1) * sizeof *rec);
+    tmp = (rk_t *)malloc((size_t)(cnt ? cnt : 1) * sizeof *tmp);
+    fill = (uint64_t *)calloc((size_t)NB, sizeof *fill);
+    if (!rec || !tmp || !fill) { free(rec); free(tmp); free(fill); return -2; }
+    for (b = 0; b <= NB; b++) offsets[b] = 0;
+    for (i = 0; i < cnt; i++) {
+        tmp[i].H = vxo_hash_pair(key, n1[i], n2[i], ns);
+        tmp[i].n1 = n1[i]; tmp[i].n2 = n2[i];
+        offsets[(tmp[i].H >> (64 - bucket_bits)) + 1]++;
+    }
+    for (b = 0; b < NB; b++) offsets[b + 1] += offsets[b];
+    for (i = 0; i < cnt; i++) {
+        b = tmp[i].H >> (64 - bucket_bits);
+        rec[offsets[b] + fill[b]++] = tmp[i];
+    }
+    for (b = 0; b < NB; b++)
+        if (offsets[b + 1] - offsets[b] > 1)
+            qsort(rec + offsets[b], (size_t)(offsets[b + 1] - offsets[b]), sizeof *rec, rk_cmp);
+    for (i = 0; i < cnt; i++) { n1_out[i] = rec[i].n1; n2_out[i] = rec[i].n2; h2_out[i] = rec[i].H; }
+    free(rec); free(tmp); free(fill);
+    return 0;
+}
+
+/* A21, the plot file: 64-byte header
+ *     "VXPLOT" 0x00 0x01 | u32 K | u32 B | u32 NONCE_SIZE | u32 0 | key[32] | u64 record count
+ * then (2^B + 1) u64 CSR offsets (in records), then the records nonce1[NONCE_SIZE] || nonce2[NONCE_SIZE]
+ * bucket-major; all integers little-endian.  Writes into out (size vxo_plot_file_bytes). */
+uint64_t vxo_plot_file_bytes(int K, int bucket_bits, uint64_t cnt)
+{
+    return 64 + 8 * ((1ULL << bucket_bits) + 1) + cnt * (uint64_t)(2 * vxo_nonce_size(K));
+}
+
+void vxo_plot_file(int K, const uint8_t key[32], int bucket_bits, uint64_t cnt, const uint64_t *offsets,
+                   const uint64_t *n1, const uint64_t *n2, uint8_t *out)
+{
+    const uint64_t NB = 1ULL << bucket_bits;
+    const int ns = vxo_nonce_size(K);
+    const uint32_t w[4] = { (uint32_t)K, (uint32_t)bucket_bits, (uint32_t)ns, 0u };
+    uint64_t b;
+    int i, j;
+    memcpy(out, "VXPLOT\0\1", 8);
+    for (i = 0; i < 4; i++) for (j = 0; j < 4; j++) out[8 + 4 * i + j] = (uint8_t)(w[i] >> (8 * j));
+    memcpy(out + 24, key, 32);
+    for (j = 0; j < 8; j++) out[56 + j] = (uint8_t)(cnt >> (8 * j));
+    for (b = 0; b <= NB; b++) for (j = 0; j < 8; j++) out[64 + 8 * b + j] = (uint8_t)(offsets[b] >> (8 * j));
+    vxo_serialize_t2(ns, cnt, n1, n2, out + 64 + 8 * (NB + 1));
 }
 
 /* ------------------------------------------------------------------ tiny CLI / timing ------- */

@@ -356,6 +356,88 @@ def test_slice_halves_and_parallel_helpers_agree_with_full_table():
     assert np.array_equal(fo, off) and np.array_equal(fn, non) and np.array_equal(fh, has)
 
 
+# ------------------------------------------------------------------ Step 6: re-keyed Table 2 (A19-A21)
+def lib_pair_hash(key: bytes, n1: int, n2: int, nsize: int) -> int:
+    """A19 with the independent `blake3` package: keyed hash of nonce1 LE || nonce2 LE, first 8 bytes BE."""
+    blake3 = pytest.importorskip("blake3")
+    msg = int(n1).to_bytes(nsize, "little") + int(n2).to_bytes(nsize, "little")
+    return int.from_bytes(blake3.blake3(msg, key=key).digest(8), "big")
+
+
+def test_pair_hash_vs_library():
+    rng = random.Random(19)
+    for seed in (1, 31, 33):
+        key = vx_inputs.key_from_seed(seed)
+        for nsize in (4, 5):
+            top = (1 << (8 * nsize)) - 1
+            cases = [(0, 0), (0, 1), (1, 0), (top, top), (top, 0), (0x01020304, 0x05060708)]
+            cases += [(rng.randrange(top + 1), rng.randrange(top + 1)) for _ in range(200)]
+            for n1, n2 in cases:
+                assert oracle.hash_pair(key, n1, n2, nsize) == lib_pair_hash(key, n1, n2, nsize)
+    # not symmetric, and not the hash of either nonce alone
+    key = vx_inputs.key_from_seed(1)
+    assert oracle.hash_pair(key, 5, 9, 4) != oracle.hash_pair(key, 9, 5, 4)
+    assert oracle.hash_pair(key, 5, 0, 4) != oracle.hash_nonce(key, 5, 4)
+
+
+@pytest.mark.parametrize("K,B,seed", [(10, 4, 3), (12, 8, 1), (14, 24, 5), (16, 12, 1)])
+def test_rekeyed_table2_vs_library_and_lexsort(K, B, seed):
+    """A20 against an independent construction: library pair hashes + numpy lexsort."""
+    key = vx_inputs.key_from_seed(seed)
+    off, non, has = oracle.table1(K, key, B)
+    t2o, n1, n2 = oracle.table2(K, off, non, has, 1)
+    ro, r1, r2, rh = oracle.table2_rekey(K, key, B, n1, n2)
+    H2 = np.array([lib_pair_hash(key, a, b, 4) for a, b in zip(n1, n2)], dtype=np.uint64)
+    order = np.lexsort((n2, n1, H2))                      # H2 major; bucket = H2 prefix, so bucket-major too
+    assert np.array_equal(r1, n1[order]) and np.array_equal(r2, n2[order]) and np.array_equal(rh, H2[order])
+    want_off = np.concatenate(([0], np.cumsum(np.bincount((H2 >> np.uint64(64 - B)).astype(np.int64),
+                                                          minlength=1 << B)))).astype(np.uint64)
+    assert np.array_equal(ro, want_off)
+    # any input order gives the same table; the pairs are a permutation of Table 2
+    perm = np.random.default_rng(seed).permutation(len(n1))
+    po, p1, p2, ph = oracle.table2_rekey(K, key, B, n1[perm], n2[perm])
+    assert np.array_equal(po, ro) and np.array_equal(p1, r1) and np.array_equal(p2, r2) and np.array_equal(ph, rh)
+    a = np.sort((n1 << np.uint64(32)) | n2)
+    b = np.sort((r1 << np.uint64(32)) | r2)
+    assert np.array_equal(a, b)
+
+
+def test_rekeyed_bucket_histogram_closed_form():
+    """Pair hashes are uniform: bucket loads of the re-keyed table ~ Poisson(|T2| / 2^B)."""
+    K, B, seed = 16, 12, 1
+    key = vx_inputs.key_from_seed(seed)
+    off, non, has = oracle.table1(K, key, B)
+    t2o, n1, n2 = oracle.table2(K, off, non, has, 1)
+    ro, r1, r2, rh = oracle.table2_rekey(K, key, B, n1, n2)
+    sizes = np.diff(ro).astype(np.int64)
+    lam = len(n1) / (1 << B)
+    hist = np.bincount(sizes)
+    for s_ in range(min(len(hist), 30)):
+        expect = (1 << B) * math.exp(-lam) * lam ** s_ / math.factorial(s_)
+        assert abs(hist[s_] - expect) < 6 * math.sqrt(expect) + 6
+    # and the re-keyed buckets are not the source buckets (the pair hash is a fresh key)
+    assert not np.array_equal(ro, t2o)
+
+
+def test_plot_file_bytes_spelled_out():
+    key = bytes(range(32))
+    offsets = np.array([0, 1, 1, 3], dtype=np.uint64)        # B = 1 would need 3 entries; use B = 1 -> 2^1 + 1 = 3
+    offsets = np.array([0, 1, 3], dtype=np.uint64)
+    n1 = np.array([0x01020304, 5, 6], dtype=np.uint64)
+    n2 = np.array([0x0a0b0c0d, 7, 8], dtype=np.uint64)
+    f = oracle.plot_file(12, key, 1, offsets, n1, n2)
+    want = (b"VXPLOT\x00\x01" + (12).to_bytes(4, "little") + (1).to_bytes(4, "little") + (4).to_bytes(4, "little")
+            + (0).to_bytes(4, "little") + key + (3).to_bytes(8, "little")
+            + b"".join(int(o).to_bytes(8, "little") for o in offsets)
+            + bytes([4, 3, 2, 1, 0x0d, 0x0c, 0x0b, 0x0a]) + (5).to_bytes(4, "little") + (7).to_bytes(4, "little")
+            + (6).to_bytes(4, "little") + (8).to_bytes(4, "little"))
+    assert bytes(f) == want
+    # 5-byte nonces
+    f5 = oracle.plot_file(33, key, 1, offsets, n1, n2)
+    assert len(f5) == 64 + 24 + 30 and bytes(f5[16:20]) == (5).to_bytes(4, "little")
+    assert bytes(f5[88:98]) == bytes([4, 3, 2, 1, 0, 0x0d, 0x0c, 0x0b, 0x0a, 0])
+
+
 def test_K24_golden_histogram_and_match_count():
     # the plain oracle needs ~15 s here; this is the largest full-table pin (mean 1 record/bucket)
     (row,) = [r for r in _rows("bucket_histograms.txt") if r[0] == "24"]
