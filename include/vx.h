@@ -138,6 +138,28 @@ vx_status vx_sort_match_table2_to_host(vx_plot *p, void *compute_stream, void *c
 vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *copy_stream, uint32_t slices,
                                        int fd, void *pinned_staging, size_t staging_bytes, uint64_t *file_bytes);
 
+/* Table-2 re-keying and the plot file (PAPER.md L49 / L77 "plot files ... searched by
+ * the ... prover", L65 the four-stage pipeline ending in the file).  Table 2 leaves the match step
+ * grouped by the bucket of the Table-1 hash; a prover looks a challenge up by the hash of the PAIR.
+ * The paper gives neither that hash nor the file layout and VaultX is unpublished (L183): readings
+ * A19-A21 of DESIGN.md are this library's own (parity with VaultX unpinned).
+ *   vx_rekey_table2   after vx_sort_match_table2*: hash every pair, H2 = first 8 bytes (big-endian) of
+ *                     the BLAKE3 keyed hash of nonce1 LE || nonce2 LE under the plot key, and bucket
+ *                     the pairs by H2 >> (64 - B), each bucket in H2 order, with CSR offsets.  The
+ *                     {H2, pair index} records are built in Table 1's partition array: TABLE 1 IS GONE
+ *                     afterwards (vx_read_tables(1) / vx_device_tables return VX_ERR_STATE), Table 2
+ *                     itself stays readable.  Enqueues only.  One-pass plots with 4-byte nonces
+ *                     (K <= 32); otherwise VX_ERR_UNSUPPORTED.
+ *   vx_read_tables(p, VX_TABLE2_REKEYED, ...)  the re-keyed buckets in the external Table-2 record
+ *                     format (the order of pairs with equal H2 is unspecified, reading A20).
+ *   vx_write_plot_file  header "VXPLOT\0\1" | u32 K | u32 B | u32 NONCE_SIZE | u32 0 | key[32] |
+ *                     u64 records, then the 2^B + 1 u64 offsets, then the records bucket-major, all
+ *                     little-endian, written to fd with sequential write()s through pinned_staging
+ *                     (HOST, >= 1 MB).  Blocks.  *file_bytes = bytes written. */
+#define VX_TABLE2_REKEYED 3
+vx_status vx_rekey_table2(vx_plot *p, void *cuda_stream);
+vx_status vx_write_plot_file(vx_plot *p, int fd, void *pinned_staging, size_t staging_bytes, uint64_t *file_bytes);
+
 /* Bucket-range passes (VI: "chunked VRAM tiling to handle k > 31
  * without requiring the full Table-1 in VRAM").  A plot with P = 2^l passes is made one hash-prefix
  * slice at a time: pass s hashes ALL 2^K nonces but keeps only the records whose top l hash bits are

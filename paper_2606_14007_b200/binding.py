@@ -18,6 +18,7 @@ VX_OPT_FORCE_EXACT_RANK = 1
 VX_OPT_PARTITION_CAPACITY_LIMIT = 2
 VX_OPT_TABLE2_CAPACITY_LIMIT = 3
 VX_OPT_SUBKEY_BITS = 4
+VX_TABLE2_REKEYED = 3
 VX_CREATE_WIDE_LAYOUT = 1
 VX_CREATE_BIG_TILES = 2
 
@@ -33,7 +34,7 @@ EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_op
            "vx_plot_create_ex", "vx_plot_create_opts",
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
            "vx_sort_match_table2_to_file", "vx_read_tables", "vx_plot_passes", "vx_plot_select_pass",
-           "vx_plot_all_passes_to_host", "vx_shard_owner", "vx_shard_begin", "vx_shard_scatter", "vx_shard_finish",
+           "vx_plot_all_passes_to_host", "vx_rekey_table2", "vx_write_plot_file", "vx_shard_owner", "vx_shard_begin", "vx_shard_scatter", "vx_shard_finish",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink", "vx_probe_alu",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
@@ -108,6 +109,10 @@ def load_library() -> ctypes.CDLL:
     L.vx_shard_scatter.argtypes = [_vp, _u32, _u32, ctypes.POINTER(_vp), _vp]
     L.vx_shard_finish.restype = ctypes.c_int
     L.vx_shard_finish.argtypes = [_vp, _vp]
+    L.vx_rekey_table2.restype = ctypes.c_int
+    L.vx_rekey_table2.argtypes = [_vp, _vp]
+    L.vx_write_plot_file.restype = ctypes.c_int
+    L.vx_write_plot_file.argtypes = [_vp, ctypes.c_int, _vp, _sz, ctypes.POINTER(_u64)]
     L.vx_read_tables.restype = ctypes.c_int
     L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
     L.vx_device_tables.restype = ctypes.c_int
@@ -277,6 +282,17 @@ class Plot:
                 self._h, self._sp(stream), self._sp(copy_stream), slices, records_ptr, records_capacity,
                 offsets_ptr or None, ctypes.byref(need), ctypes.byref(t1)))
         return need.value, t1.value
+
+    # -- re-keying + plot file (8(f2)) -------------------------------------------------------------
+    def rekey_table2(self, stream=None):
+        with self._dev():
+            self._check(self._L.vx_rekey_table2(self._h, self._sp(stream)))
+
+    def write_plot_file(self, fd: int, staging_ptr: int, staging_bytes: int) -> int:
+        n = _u64()
+        with self._dev():
+            self._check(self._L.vx_write_plot_file(self._h, fd, staging_ptr, staging_bytes, ctypes.byref(n)))
+        return n.value
 
     # -- one plot over G GPUs (8(f4)) ------------------------------------------------------------
     def shard_begin(self, rank: int, world: int, stream=None):

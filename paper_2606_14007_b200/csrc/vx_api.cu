@@ -13,11 +13,12 @@
 #include "../../include/vx.h"
 #include "vx_internal.h"
 
-enum VxState { VX_CREATED = 0, VX_BOUND = 1, VX_BUILT = 2, VX_MATCHED = 3 };
+enum VxState { VX_CREATED = 0, VX_BOUND = 1, VX_BUILT = 2, VX_MATCHED = 3, VX_REKEYED = 4 };
 
 struct vx_plot {
     VxGeom g;
     VxHashConst hc;
+    VxHashConst hc2;        // the same key with block_len = 2 NONCE_SIZE: the pair hash of the re-keying (A19)
     uint8_t key[32];
     uint8_t *ws;
     size_t ws_bytes;
@@ -238,6 +239,7 @@ vx_status vx_plot_create_opts(uint32_t K, const uint8_t key[32], uint32_t bucket
     p->g = g;
     memcpy(p->key, key, 32);
     vx_hash_const_init(&p->hc, key, g.nonce_size);
+    vx_hash_const_init(&p->hc2, key, 2 * g.nonce_size);
     p->state = VX_CREATED;
     snprintf(p->err, sizeof p->err, "VX_OK");
     *out = p;
@@ -323,10 +325,14 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
                          size_t *records_bytes)
 {
     if (!p) return VX_ERR_ARG;
-    if (table != 1 && table != 2) return fail(p, VX_ERR_ARG, "table must be 1 or 2");
+    if (table != 1 && table != 2 && table != VX_TABLE2_REKEYED) return fail(p, VX_ERR_ARG, "table must be 1, 2 or VX_TABLE2_REKEYED");
     if (p->state < VX_BUILT) return fail(p, VX_ERR_STATE, "vx_read_tables before vx_build_table1");
     if (table == 2 && p->state < VX_MATCHED)
         return fail(p, VX_ERR_STATE, "Table 2 read before vx_sort_match_table2");
+    if (table == VX_TABLE2_REKEYED && p->state < VX_REKEYED)
+        return fail(p, VX_ERR_STATE, "re-keyed Table 2 read before vx_rekey_table2");
+    if (table == 1 && p->state >= VX_REKEYED)
+        return fail(p, VX_ERR_STATE, "Table 1 was overwritten by vx_rekey_table2 (its partition array holds the pair hashes now)");
     if (bucket_begin > bucket_end || bucket_end > p->g.NB)
         return fail(p, VX_ERR_RANGE, "bucket range outside [0, 2^B]");
     if (bucket_begin < p->g.b_first || bucket_end > p->g.b_first + p->g.NBp)
@@ -341,7 +347,8 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
     }
     vx_status s = sync_and_check(p);
     if (s != VX_OK) return s;
-    const uint8_t *off_dev = p->ws + (table == 1 ? p->g.off_t1_off : p->g.off_t2_off);
+    // (the re-keyed table's CSR offsets were written where Table 1's were)
+    const uint8_t *off_dev = p->ws + (table == 2 ? p->g.off_t2_off : p->g.off_t1_off);
     const size_t rb = table == 1 ? p->g.rec1_bytes : p->g.rec2_bytes;
     const uint64_t nb = bucket_end - bucket_begin;
     uint64_t first = 0, last = 0;
@@ -364,6 +371,20 @@ vx_status vx_read_tables(vx_plot *p, int table, uint64_t bucket_begin, uint64_t 
         for (uint64_t done = 0; done < last - first; done += per2) {
             const uint64_t n = (last - first - done) < per2 ? (last - first - done) : per2;
             e = vx_launch_export_t2(p->g, p->ws, first + done, n, p->stream);
+            if (e != cudaSuccess) return fail_cuda(p, e, "export launch");
+            e = cudaMemcpyAsync((uint8_t *)records_out + done * rb, p->ws + p->g.off_stage, n * rb,
+                                cudaMemcpyDeviceToHost, p->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+            if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(exported records)");
+        }
+        return VX_OK;
+    }
+    if (table == VX_TABLE2_REKEYED) {
+        // gather the pairs in H2 order through the sorted pair indices, a staging chunk at a time
+        const uint64_t per3 = p->g.stage_bytes / rb;
+        for (uint64_t done = 0; done < last - first; done += per3) {
+            const uint64_t n = (last - first - done) < per3 ? (last - first - done) : per3;
+            e = vx_launch_export_rekey(p->g, p->ws, first + done, n, p->stream);
             if (e != cudaSuccess) return fail_cuda(p, e, "export launch");
             e = cudaMemcpyAsync((uint8_t *)records_out + done * rb, p->ws + p->g.off_stage, n * rb,
                                 cudaMemcpyDeviceToHost, p->stream);
@@ -461,6 +482,69 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
     }
     if (file_bytes) *file_bytes = written;
     return s;
+}
+
+// ------------------------------------------------------------------------------ re-keying + plot file (8(f2))
+vx_status vx_rekey_table2(vx_plot *p, void *cuda_stream)
+{
+    if (!p) return VX_ERR_ARG;
+    if (p->state < VX_MATCHED) return fail(p, VX_ERR_STATE, "vx_rekey_table2 before vx_sort_match_table2");
+    if (p->state >= VX_REKEYED) return fail(p, VX_ERR_STATE, "Table 2 is already re-keyed");
+    if (p->g.wide || p->g.passes_log)
+        return fail(p, VX_ERR_UNSUPPORTED, "re-keying is implemented for one-pass plots in the 16-byte record layout (K <= 32)");
+    p->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = vx_launch_rekey(p->g, p->hc2, p->ws, p->stream);
+    if (e == cudaSuccess) e = vx_launch_stage2(p->g, p->ws, false, p->force_exact, p->num_sms, p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e, "re-keying launch");
+    p->state = VX_REKEYED;
+    p->t1_materialised = true;                             // the bucket view in the workspace is the re-keyed table's
+    return VX_OK;
+}
+
+vx_status vx_write_plot_file(vx_plot *p, int fd, void *pinned_staging, size_t staging_bytes, uint64_t *file_bytes)
+{
+    if (!p) return VX_ERR_ARG;
+    if (file_bytes) *file_bytes = 0;
+    if (fd < 0 || !pinned_staging || staging_bytes < ((size_t)1 << 20))
+        return fail(p, VX_ERR_ARG, "bad file descriptor, or staging buffer NULL / smaller than 1 MB");
+    if (p->state < VX_REKEYED) return fail(p, VX_ERR_STATE, "vx_write_plot_file before vx_rekey_table2");
+    vx_status s = sync_and_check(p);
+    if (s != VX_OK) return s;
+    VxCtrl c;
+    cudaError_t e = cudaMemcpy(&c, p->ws + p->g.off_ctrl, sizeof c, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(ctrl)");
+    const uint64_t M = c.t2_total;
+    uint64_t written = 0;
+    char msg[128];
+    // header (reading A21): magic, K, B, NONCE_SIZE, 0, key, record count
+    uint8_t hd[64] = {'V', 'X', 'P', 'L', 'O', 'T', 0, 1};
+    const uint32_t w[4] = {p->g.K, p->g.B, p->g.nonce_size, 0u};
+    memcpy(hd + 8, w, 16);
+    memcpy(hd + 24, p->key, 32);
+    memcpy(hd + 56, &M, 8);
+    if (vx_write_all(fd, hd, sizeof hd, &written, msg, sizeof msg)) return fail(p, VX_ERR_IO, msg);
+    uint8_t *host = (uint8_t *)pinned_staging;
+    // CSR offsets, then the records in H2 order (gathered on the device a staging chunk at a time)
+    const uint8_t *off_dev = p->ws + p->g.off_t1_off;
+    const size_t off_bytes = (p->g.NB + 1) * 8;
+    for (size_t at = 0; at < off_bytes; at += staging_bytes) {
+        const size_t n = off_bytes - at < staging_bytes ? off_bytes - at : staging_bytes;
+        e = cudaMemcpy(host, off_dev + at, n, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(offsets)");
+        if (vx_write_all(fd, host, n, &written, msg, sizeof msg)) { if (file_bytes) *file_bytes = written; return fail(p, VX_ERR_IO, msg); }
+    }
+    const size_t rb = p->g.rec2_bytes;
+    size_t chunk = (p->g.stage_bytes < staging_bytes ? p->g.stage_bytes : staging_bytes) / rb;
+    for (uint64_t done = 0; done < M; done += chunk) {
+        const uint64_t n = M - done < chunk ? M - done : chunk;
+        e = vx_launch_export_rekey(p->g, p->ws, done, n, p->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(host, p->ws + p->g.off_stage, n * rb, cudaMemcpyDeviceToHost, p->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+        if (e != cudaSuccess) return fail_cuda(p, e, "export of the re-keyed records");
+        if (vx_write_all(fd, host, n * rb, &written, msg, sizeof msg)) { if (file_bytes) *file_bytes = written; return fail(p, VX_ERR_IO, msg); }
+    }
+    if (file_bytes) *file_bytes = written;
+    return VX_OK;
 }
 
 // ------------------------------------------------------------------------------ passes (8(f3))
@@ -598,6 +682,7 @@ vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64
 {
     if (!p) return VX_ERR_ARG;
     if (p->state < VX_MATCHED) return fail(p, VX_ERR_STATE, "vx_device_tables before vx_sort_match_table2");
+    if (p->state >= VX_REKEYED) return fail(p, VX_ERR_STATE, "vx_device_tables after vx_rekey_table2 (Table 1 is gone)");
     if (dev_t1_records) *dev_t1_records = p->ws + p->g.off_part;
     if (dev_t1_offsets) *dev_t1_offsets = (const uint64_t *)(p->ws + p->g.off_t1_off);
     if (dev_t2_records) *dev_t2_records = p->ws + p->g.off_t2_rec;
@@ -639,7 +724,7 @@ vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, u
     uint64_t t1 = 0;
     e = cudaMemcpy(&t1, p->ws + p->g.off_part_base + p->g.P * 8, 8, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemcpy(part_base)");
-    if (t1_records) *t1_records = t1;
+    if (t1_records) *t1_records = p->state >= VX_REKEYED ? c.t1_total : t1;
     if (t2_records) *t2_records = p->state >= VX_MATCHED ? c.t2_total : 0;
     if (max_bucket) *max_bucket = p->t1_materialised ? c.max_bucket : 0;
     return VX_OK;

@@ -76,7 +76,7 @@ struct VxCtrl {
     uint32_t max_bucket;  // largest Table-1 bucket seen by stage 2
     uint32_t retries;     // tiles that stage 2 re-ranked exactly after its fast ranking met a tie
     unsigned long long t2_total;  // number of Table-2 records
-    unsigned long long pad1;
+    unsigned long long t1_total;  // Table-1 records, saved by vx_rekey_table2 before the partition bases are rebuilt
 };
 #define VX_FLAG_PART_OVERFLOW 1u
 #define VX_FLAG_T2_OVERFLOW 2u
@@ -113,6 +113,13 @@ cudaError_t vx_launch_shard_clear(const VxGeom &g, uint8_t *ws, cudaStream_t st)
 cudaError_t vx_launch_shard_scatter(const VxGeom &g, const VxHashConst &hc, uint32_t rank, uint32_t world_log,
                                     uint8_t *const *peer_ws, cudaStream_t st);
 cudaError_t vx_launch_shard_scan(const VxGeom &g, uint8_t *ws, cudaStream_t st);
+// Table-2 re-keying (8(f2)): hash every pair (hc2: block_len = 2 NONCE_SIZE), append {H2, pair index}
+// to the hash-prefix partitions (the partition array of Table 1 is reused), scan.  Then
+// vx_launch_stage2(do_match = false) sorts the partitions and writes the CSR offsets.
+cudaError_t vx_launch_rekey(const VxGeom &g, const VxHashConst &hc2, uint8_t *ws, cudaStream_t st);
+// re-keyed pairs [first, first + count) of the CSR numbering, gathered through the sorted pair indices
+// into the external Table-2 format in ws + off_stage
+cudaError_t vx_launch_export_rekey(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st);
 // zero two regions and two words with a kernel (not a memset: see vx_k_clear)
 cudaError_t vx_launch_clear(cudaStream_t st, void *a, size_t bytes_a, void *b, size_t bytes_b, uint32_t *w0, uint32_t *w1);
 // sorts (and matches) the partitions [tile_begin, tile_end) -- (0, P) for the whole plot; slices must

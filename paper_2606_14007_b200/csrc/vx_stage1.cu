@@ -357,6 +357,74 @@ cudaError_t vx_launch_hash_sink(const VxGeom &g, const VxHashConst &hc, uint64_t
     return cudaGetLastError();
 }
 
+// ----------------------------------------------------------------------------- Table-2 re-keying (8(f2))
+// SURVEY.md 8(f2) / PAPER.md L49, L65, L77: a prover looks a challenge up by hash, but Table 2 leaves
+// the match step grouped by the bucket of the TABLE-1 hash.  Readings A19/A20: every pair
+// is hashed, H2 = BLAKE3 keyed hash of nonce1 || nonce2 (the same compression as stage 1 with message
+// words m0 = n1, m1 = n2 and block_len 8), and the pairs are bucketed by H2 exactly as stage 1 buckets
+// nonces: atomic append of {H2, index of the pair in Table 2} into the coarse hash-prefix partitions
+// -- the partition array of Table 1, which has done its job -- then the fused kernel sorts every
+// partition (no matching) and writes the CSR offsets.  The pairs themselves stay where they are; the
+// export gathers them in H2 order.
+__global__ void __launch_bounds__(VX_S1_THREADS)
+vx_k_rekey_scatter(const __grid_constant__ VxHashConst hc2, const uint2 *__restrict__ t2_rec, uint32_t pb,
+                   uint32_t cap, uint32_t cap_check, uint4 *__restrict__ part, uint32_t *__restrict__ cursor,
+                   VxCtrl *__restrict__ ctrl)
+{
+    const unsigned long long M = ctrl->t2_total;
+    const uint64_t base = (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
+    if ((uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) >= M) return;
+    if (M > 0xffffffffull) {                            // the pair index is kept in 32 bits
+        if (base == 0) atomicOr(&ctrl->flags, VX_FLAG_T2_OVERFLOW);
+        return;
+    }
+    uint64_t H[VX_S1_NPT];
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t r = base + (uint64_t)k * VX_S1_THREADS;
+        const uint2 pr = r < M ? __ldcs(t2_rec + r) : make_uint2(0u, 0u);
+        H[k] = vx_blake3_h<true>(hc2, pr.x, pr.y);
+    }
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t r = base + (uint64_t)k * VX_S1_THREADS;
+        if (r < M) {
+            const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
+            const uint32_t slot = atomicAdd(&cursor[p], 1u);
+            if (slot < cap_check)
+                part[(uint64_t)p * cap + slot] = make_uint4((uint32_t)H[k], (uint32_t)(H[k] >> 32), (uint32_t)r, 0u);
+            else
+                atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
+        }
+    }
+}
+
+// the Table-1 record count, kept for vx_get_stats before the partition bases are rebuilt for the pairs
+__global__ void vx_k_save_t1_total(const unsigned long long *__restrict__ part_base, uint64_t P, VxCtrl *__restrict__ ctrl)
+{
+    ctrl->t1_total = part_base[P];
+}
+
+cudaError_t vx_launch_rekey(const VxGeom &g, const VxHashConst &hc2, uint8_t *ws, cudaStream_t st)
+{
+    if (g.wide || g.passes_log) return cudaErrorInvalidValue;
+    VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
+    uint32_t *cursor = (uint32_t *)(ws + g.off_cursor);
+    vx_k_save_t1_total<<<1, 1, 0, st>>>((const unsigned long long *)(ws + g.off_part_base), g.P, ctrl);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = vx_launch_clear(st, cursor, g.P * sizeof(uint32_t), nullptr, 0, nullptr, nullptr);
+    if (e != cudaSuccess) return e;
+    const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
+    const uint64_t grid = (g.t2_cap + per_cta - 1) / per_cta;          // upper bound; CTAs beyond |Table 2| exit
+    vx_k_rekey_scatter<<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc2, (const uint2 *)(ws + g.off_t2_rec), g.pb, g.cap,
+                                                                 g.cap_check, (uint4 *)(ws + g.off_part), cursor, ctrl);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap_check, g.P,
+                                                       (unsigned long long *)(ws + g.off_part_base));
+    return cudaGetLastError();
+}
+
 // ----------------------------------------------------------------------------- one plot over G GPUs: launches
 cudaError_t vx_launch_shard_clear(const VxGeom &g, uint8_t *ws, cudaStream_t st)
 {

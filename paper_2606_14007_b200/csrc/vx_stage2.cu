@@ -602,6 +602,38 @@ vx_k_export_t2(const uint2 *__restrict__ rec, const uint8_t *__restrict__ hi, un
     }
 }
 
+// re-keyed Table 2 (8(f2)): the partition array holds {H2, pair index} sorted by H2; records
+// [first, first + count) of its CSR numbering are the pairs t2_rec[index], gathered here.
+__global__ void __launch_bounds__(256)
+vx_k_export_rekey(const uint4 *__restrict__ part, const unsigned long long *__restrict__ part_base, uint32_t P,
+                  uint32_t cap, const uint2 *__restrict__ t2_rec, unsigned long long first,
+                  unsigned long long count, uint2 *__restrict__ out)
+{
+    for (unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; r < count;
+         r += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long g = first + r;
+        uint32_t lo = 0, hi = P;
+        while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (part_base[mid] <= g) lo = mid; else hi = mid;
+        }
+        const uint4 rec = part[(size_t)lo * cap + (g - part_base[lo])];
+        out[r] = t2_rec[rec.z];
+    }
+}
+
+cudaError_t vx_launch_export_rekey(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st)
+{
+    if (count == 0) return cudaSuccess;
+    uint64_t grid = (count + 255) / 256;
+    if (grid > (uint64_t)vx_sm_count() * 16) grid = (uint64_t)vx_sm_count() * 16;
+    vx_k_export_rekey<<<(unsigned)grid, 256, 0, st>>>((const uint4 *)(ws + g.off_part),
+                                                      (const unsigned long long *)(ws + g.off_part_base), (uint32_t)g.P,
+                                                      g.cap, (const uint2 *)(ws + g.off_t2_rec), first, count,
+                                                      (uint2 *)(ws + g.off_stage));
+    return cudaGetLastError();
+}
+
 cudaError_t vx_launch_export_t1(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count,
                                 cudaStream_t st)
 {
