@@ -252,10 +252,10 @@ vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64
  * synchronising call instead of dropping records silently (reading A8). */
 #define VX_OPT_PARTITION_CAPACITY_LIMIT 2
 #define VX_OPT_TABLE2_CAPACITY_LIMIT 3
-/* VX_OPT_SUBKEY_BITS (0 .. 32, default 32; 31 and above mean all 31 the kernel keeps): how many hash
+/* VX_OPT_SUBKEY_BITS (0 .. 32, default 32; 28 and above mean all 28 the kernel keeps): how many hash
  * bits below the bin index the fused kernel's fast in-bin ranking compares.  Fewer bits make records of one bin tie, come out in the wrong order
- * and so send the tile through its "redo with exact (H, n) ranks" path (taken about once per 2^20
- * tiles otherwise) -- results are identical by construction; tests use it to run that path. */
+ * and so send the tile through its "redo with exact (H, n) ranks" path (taken by about 8 tiles of
+ * a K = 31 plot otherwise) -- results are identical by construction; tests use it to run that path. */
 #define VX_OPT_SUBKEY_BITS 4
 vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value);
 
@@ -264,7 +264,7 @@ vx_status vx_get_stats(vx_plot *p, uint64_t *t1_records, uint64_t *t2_records, u
 
 /* Synchronises.  tile_retries = tiles of the last stage 2 whose fast in-bin ranking met a tie (two
  * records of a bin with equal compared sub-keys, among them equal 64-bit hashes, reading A10) and
- * which were therefore re-ranked by exact (H, n) compares; ~2^-21 per tile at the default 32
+ * which were therefore re-ranked by exact (H, n) compares; about 2^-16 per tile at the default
  * sub-key bits.  For tests of that path (VX_OPT_SUBKEY_BITS). */
 vx_status vx_get_counters(vx_plot *p, uint64_t *tile_retries);
 

@@ -145,13 +145,13 @@ vx_lookback(unsigned long long *status, uint32_t tile, unsigned long long aggreg
     return excl;
 }
 
-// the 31 hash bits right below the bin index (bin = (H >> binshift) & (VX_NBINS - 1)), as a value
-// below 2^31 (so that sub-key + 1 never wraps, see the ranking pass).  binshift >= 32 always
-// (pb + VX_BIN_BITS <= 32; checked at launch), so both are 32-bit operations on the high word:
+// the 32 hash bits right below the bin index (bin = (H >> binshift) & (VX_NBINS - 1)); the caller masks
+// off the low 4 (the record's slot in its bin goes there) and whatever a test hook narrows.  binshift >= 32
+// always (pb + VX_BIN_BITS <= 32; checked at launch), so both are 32-bit operations on the high word:
 // sh = binshift - 32
 __device__ __forceinline__ uint32_t vx_subkey(uint64_t k, int sh)
 {
-    return __funnelshift_r((uint32_t)k, (uint32_t)(k >> 32), sh) >> 1;
+    return __funnelshift_r((uint32_t)k, (uint32_t)(k >> 32), sh);
 }
 template <uint32_t NBINS>
 __device__ __forceinline__ uint32_t vx_bin(uint64_t k, int sh)
@@ -199,7 +199,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     // the predecessors get that much longer to publish their totals.
     const bool defer = q.do_match && nb_local <= VX_DEFER_MAXB;
     bool pending = false;                               // CTA-uniform
-    uint32_t p_tile = 0, p_cnt = 0, p_M = 0;
+    // (tile, count and matches of the tile whose emit is pending: CTA-uniform, so they live in shared
+    // memory rather than in three registers of every thread -- the kernel sits at its register limit)
+    __shared__ uint32_t s_p[3];
 
     // ---- look-back for the Table-2 base, then H: the matches of i are i+1 .. i+c_i, c_i = E[i+1] - E[i]
     auto lookback_emit = [&](uint32_t tile, uint32_t cnt, uint32_t M) {
@@ -278,7 +280,6 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         // validated in phase E (a tile holding two equal hashes comes back for an exact pass)
         uint32_t exact = q.force_exact | (q.do_match ^ 1u);
         uint32_t tile, cnt;
-        unsigned long long base1;
         uint4 *src;
         unsigned short *src_b = nullptr;
         uint64_t key[ITEMS];
@@ -293,7 +294,6 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             tile = s_tile;
             const bool valid = tile < q.tile_end;
             cnt = valid ? min(q.cursor[tile], q.cap_check) : 0u;
-            base1 = valid ? q.part_base[tile] : 0ull;
             if constexpr (WIDE) {
                 src = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned long long *>(q.part) + (size_t)tile * q.cap);
                 src_b = q.part_b + (size_t)tile * q.cap;
@@ -321,7 +321,8 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin<VX_NBINS>(key[it], sh)], 1u);
             }
             if (pending) {                              // the previous tile of this CTA: look-back + H
-                const unsigned long long base2 = lookback_emit(p_tile, p_cnt, p_M);
+                const uint32_t p_tile = s_p[0], p_M = s_p[2];
+                const unsigned long long base2 = lookback_emit(p_tile, s_p[1], p_M);
                 const unsigned long long pg0 = (unsigned long long)p_tile << q.fb;
                 for (uint32_t bl = tid; bl < nb_local; bl += THREADS) q.t2_off[pg0 + bl] = base2 + s_e2[bl];
                 if (p_tile == q.P - 1 && tid == 0) {
@@ -349,7 +350,11 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                         VX_CHECK(q.ctrl, pos < cnt);
                         keyS[pos] = key[it];
                         nonS[pos] = non[it];
-                        sub[pos] = vx_subkey(key[it], sh) & submask;
+                        // ranking key: the hash bits below the bin index with the record's slot in the bin
+                        // (its arrival order, unique there) in the low 4 bits -- distinct within a bin, so the
+                        // ranks below are distinct and no two lanes ever write one sorted slot
+                        sub[pos] = (vx_subkey(key[it], sh) & submask) | sn[it];
+                        if (sn[it] > 15u) s_tie = 1u;   // a bin of more than 16 records: rank it exactly
                     }
                 }
             }
@@ -371,25 +376,22 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t nm = __reduce_max_sync(VX_FULL, n);
                     uint32_t rank = 0;
                     if (!exact) {
-                        // by (the 32 bits below the bin index, position in the bin): every record of a
-                        // bin gets a rank of its own, so no two lanes ever write one slot.  Records
-                        // with equal sub-keys (or equal hashes) may come out in the wrong order, which
-                        // phase E sees as keys that do not strictly increase
+                        // by the ranking key of phase C: (27 hash bits below the bin index, slot in the bin).
+                        // Every record of a bin gets a rank of its own.  Records that tie on those hash bits
+                        // may come out in the wrong order, which phase E sees as keys that do not strictly
+                        // increase (about 8 tiles of a K = 31 plot), as it does two equal hashes
                         const uint32_t *sp = sub + s;
-                        const uint32_t ks = sub[i];                         // < 2^31
-                        const uint32_t me = i - s;
-                        // (kj, j) < (ks, me)  <=>  kj < ks + (j < me); the own slot and the slots
-                        // beyond the bin (sentinel ~0) never count
+                        const uint32_t ks = sub[i];
 #pragma unroll
                         for (uint32_t j = 0; j < 4; j++) {
                             const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
-                            rank += kj < ks + (j < me ? 1u : 0u) ? 1u : 0u;
+                            rank += kj < ks ? 1u : 0u;
                         }
                         if (nm > 4) {
 #pragma unroll 1
                             for (uint32_t j = 4; j < nm; j++) {
                                 const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
-                                rank += kj < ks + (j < me ? 1u : 0u) ? 1u : 0u;
+                                rank += kj < ks ? 1u : 0u;
                             }
                         }
                     } else {                            // by (H, n), reading A10
@@ -511,6 +513,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             }
         }
         const unsigned long long gb0 = (unsigned long long)tile << q.fb;
+        const unsigned long long base1 = q.part_base[tile];
         for (uint32_t bl = tid; bl < nb_local; bl += THREADS) {
             const uint32_t s = bucket_start(bl), e = bucket_start(bl + 1);
             VX_CHECK(q.ctrl, s <= e && e <= cnt && gb0 + bl < q.NB && (!defer || bl < VX_DEFER_MAXB));
@@ -522,7 +525,8 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
 
         if (q.do_match) {
             if (defer) {
-                pending = true; p_tile = tile; p_cnt = cnt; p_M = M;
+                pending = true;
+                if (tid == 0) { s_p[0] = tile; s_p[1] = cnt; s_p[2] = M; }   // read behind the next tile's barriers
             } else {
                 const unsigned long long base2 = lookback_emit(tile, cnt, M);
                 for (uint32_t bl = tid; bl < nb_local; bl += THREADS)
@@ -714,7 +718,8 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     q.P = (uint32_t)g.P; q.cap = g.cap; q.cap_check = g.cap_check; q.pb = g.pb; q.fb = g.fb; q.K = g.K; q.B = g.B;
     q.do_match = do_match ? 1u : 0u;
     q.force_exact = force_exact ? 1u : 0u;
-    q.submask = g.subkey_bits >= 31 ? 0x7fffffffu : (0x7fffffffu >> (31 - g.subkey_bits)) << (31 - g.subkey_bits);
+    // 28 hash bits at most: the low 4 bits of the ranking key hold the record's slot in its bin
+    q.submask = g.subkey_bits >= 28 ? 0xfffffff0u : g.subkey_bits == 0 ? 0u : ~0u << (32 - g.subkey_bits);
     q.tile_begin = tile_begin; q.tile_end = tile_end; q.slice_end_out = slice_end_out;
     if (g.pb + g.tile_log > 32 && !g.wide) return cudaErrorInvalidValue;   // bin and sub-key sit in the high word
     q.part_b = (uint16_t *)(ws + g.off_part_b);
