@@ -84,6 +84,8 @@ class ClockSampler:
     def __init__(self, index: int):
         self.index = index
         self.rows = []
+        self.when = []
+        self.t_mark = 0.0
         self.proc = None
 
     def start(self):
@@ -100,6 +102,15 @@ class ClockSampler:
     def _pump(self):
         for line in self.proc.stdout:
             self.rows.append(line.strip())
+            self.when.append(time.perf_counter())     # a line is printed right after its sample is taken
+
+    def mark(self):
+        """Samples before this moment are dropped (the sampler is started ahead of the timed region so
+        that nvidia-smi's start-up does not eat a short run)."""
+        self.t_mark = time.perf_counter()
+
+    def count(self):
+        return sum(1 for t in self.when if t >= self.t_mark)
 
     def stop(self):
         if not self.proc:
@@ -111,7 +122,9 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        for r, t in zip(self.rows, self.when):
+            if t < self.t_mark:
+                continue
             parts = [x.strip() for x in r.split(",")]
             if len(parts) < 7:
                 continue
@@ -310,6 +323,9 @@ def run_cuda(args):
             plot.sort_match_table2(stream)
             if evs: evs[3 * s + 2].record(stream)
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()                 # ahead of the warm-up: nvidia-smi needs a moment to print its first line
     for _ in range(args.warmup):
         step()
     barrier()
@@ -317,10 +333,8 @@ def run_cuda(args):
 
     # ---- device-timed region -------------------------------------------------------------
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3 * passes)] for _ in range(args.steps)]
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     barrier()
+    sampler.mark()                      # only samples taken from here on count
     for i in range(args.steps):
         step(evs[i])
     barrier()
@@ -329,7 +343,7 @@ def run_cuda(args):
     extra = 0
     if rank == 0:
         t_end = time.perf_counter() + 3.0
-        while len(sampler.rows) < 3 and time.perf_counter() < t_end:
+        while sampler.count() < 3 and time.perf_counter() < t_end:
             step(); extra += 1
             torch.cuda.synchronize()
     clocks = sampler.stop() if rank == 0 else None
