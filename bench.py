@@ -330,6 +330,7 @@ def run_cuda(args):
         step()
     barrier()
     stats = plot.get_stats()
+    stats.update(plot.get_counters())   # tiles of the last stage 2 that took the exact re-rank
 
     # ---- device-timed region -------------------------------------------------------------
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3 * passes)] for _ in range(args.steps)]
