@@ -87,7 +87,7 @@ FULL_CASES = [
 ]
 
 
-@pytest.mark.parametrize("K,B,seed", FULL_CASES)
+@pytest.mark.parametrize("K,B,seed", FULL_CASES + [(13, 4, 11), (15, 8, 12), (17, 8, 13), (19, 10, 14), (20, 12, 15), (23, 20, 16)])
 def test_tables_bit_exact_vs_oracle(vx, K, B, seed):
     key = vx_inputs.key_from_seed(seed)
     o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
