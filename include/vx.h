@@ -208,6 +208,15 @@ vx_status vx_shard_begin(vx_plot *p, uint32_t rank, uint32_t world, void *cuda_s
 vx_status vx_shard_scatter(vx_plot *p, uint32_t rank, uint32_t world, void *const *dev_peer_workspaces,
                            void *cuda_stream);
 vx_status vx_shard_finish(vx_plot *p, void *cuda_stream);
+/* Peer mapping when the ranks are separate processes (one per GPU under torch.distributed.run):
+ *   vx_ipc_export  the bound workspace as a CUDA IPC handle (64 bytes, HOST) of the cudaMalloc allocation
+ *                  it lies in plus its byte offset there (PyTorch's allocator sub-allocates);
+ *   vx_ipc_open    in ANOTHER process: map that allocation on the current device (peer access is enabled
+ *                  lazily) -> *dev_workspace for the peer table of vx_shard_scatter, *dev_mapped_base for
+ *   vx_ipc_close.  The handles travel by whatever the caller has (torch.distributed.all_gather_object). */
+vx_status vx_ipc_export(vx_plot *p, uint8_t handle[64], uint64_t *offset);
+vx_status vx_ipc_open(const uint8_t handle[64], uint64_t offset, void **dev_mapped_base, void **dev_workspace);
+vx_status vx_ipc_close(void *dev_mapped_base);
 
 /* Copy the buckets [bucket_begin, bucket_end) of table 1 or 2 to HOST memory in the external
  * format.  Synchronises the plot's stream.  offsets_out (may be NULL) receives

@@ -35,6 +35,7 @@ EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_op
            "vx_plot_bind", "vx_build_table1", "vx_sort_match_table2", "vx_sort_match_table2_to_host",
            "vx_sort_match_table2_to_file", "vx_read_tables", "vx_plot_passes", "vx_plot_select_pass",
            "vx_plot_all_passes_to_host", "vx_rekey_table2", "vx_write_plot_file", "vx_shard_owner", "vx_shard_begin", "vx_shard_scatter", "vx_shard_finish",
+           "vx_ipc_export", "vx_ipc_open", "vx_ipc_close",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
            "vx_hash_sink", "vx_probe_alu",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
@@ -113,6 +114,12 @@ def load_library() -> ctypes.CDLL:
     L.vx_rekey_table2.argtypes = [_vp, _vp]
     L.vx_write_plot_file.restype = ctypes.c_int
     L.vx_write_plot_file.argtypes = [_vp, ctypes.c_int, _vp, _sz, ctypes.POINTER(_u64)]
+    L.vx_ipc_export.restype = ctypes.c_int
+    L.vx_ipc_export.argtypes = [_vp, ctypes.c_char_p, ctypes.POINTER(_u64)]
+    L.vx_ipc_open.restype = ctypes.c_int
+    L.vx_ipc_open.argtypes = [ctypes.c_char_p, _u64, ctypes.POINTER(_vp), ctypes.POINTER(_vp)]
+    L.vx_ipc_close.restype = ctypes.c_int
+    L.vx_ipc_close.argtypes = [_vp]
     L.vx_read_tables.restype = ctypes.c_int
     L.vx_read_tables.argtypes = [_vp, ctypes.c_int, _u64, _u64, _vp, _vp, _sz, ctypes.POINTER(_sz)]
     L.vx_device_tables.restype = ctypes.c_int
@@ -304,6 +311,14 @@ class Plot:
         with self._dev():
             self._check(self._L.vx_shard_scatter(self._h, rank, world, arr, self._sp(stream)))
 
+    def ipc_export(self):
+        """(64-byte CUDA IPC handle, offset) of the workspace, for a peer process (vx_ipc_export)."""
+        buf = ctypes.create_string_buffer(64)
+        off = _u64()
+        with self._dev():
+            self._check(self._L.vx_ipc_export(self._h, buf, ctypes.byref(off)))
+        return buf.raw, off.value
+
     def shard_finish(self, stream=None):
         with self._dev():
             self._check(self._L.vx_shard_finish(self._h, self._sp(stream)))
@@ -388,6 +403,21 @@ def probe_alu(kind: str, iters: int, scratch, ctas_per_sm: int = 8, stream=None)
     if st != VX_OK:
         raise VxError(st, f"vx_probe_alu({kind})")
     return ops.value
+
+
+def ipc_open(handle: bytes, offset: int):
+    """Map a peer process's workspace (vx_ipc_open) on the current device: (mapped base, workspace pointer)."""
+    base, ws = _vp(), _vp()
+    st = load_library().vx_ipc_open(handle, offset, ctypes.byref(base), ctypes.byref(ws))
+    if st != VX_OK:
+        raise VxError(st, "vx_ipc_open")
+    return base.value, ws.value
+
+
+def ipc_close(mapped_base: int):
+    st = load_library().vx_ipc_close(mapped_base)
+    if st != VX_OK:
+        raise VxError(st, "vx_ipc_close")
 
 
 def shard_owner(K: int, bucket_bits: int, world: int, rank: int):

@@ -1,5 +1,6 @@
 // vx_api.cu -- the C ABI of libvx (include/vx.h): host-side state machine, workspace plan,
 // launches and read-back.  No device memory is allocated here: the workspace is the caller's.
+#include <dlfcn.h>
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -674,6 +675,53 @@ vx_status vx_shard_finish(vx_plot *p, void *cuda_stream)
     p->state = VX_BUILT;
     p->t1_materialised = false;
     return VX_OK;
+}
+
+// Peer mapping for ranks that are separate PROCESSES (one per GPU under torch.distributed.run): the
+// bound workspace is exported as a CUDA IPC handle of the allocation it lies in plus its offset there
+// (PyTorch's caching allocator hands out pieces of larger cudaMalloc blocks), and a peer maps it.
+typedef int (*vx_cuMemGetAddressRange_t)(unsigned long long *, size_t *, unsigned long long);
+
+vx_status vx_ipc_export(vx_plot *p, uint8_t handle[64], uint64_t *offset)
+{
+    if (!p || !handle || !offset) return VX_ERR_ARG;
+    if (p->state < VX_BOUND) return fail(p, VX_ERR_STATE, "vx_ipc_export before vx_plot_bind");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+    // the base of the allocation: driver API, resolved at run time (libvx does not link libcuda)
+    void *drv = dlopen("libcuda.so.1", RTLD_LAZY | RTLD_LOCAL);
+    vx_cuMemGetAddressRange_t range = drv ? (vx_cuMemGetAddressRange_t)dlsym(drv, "cuMemGetAddressRange_v2") : NULL;
+    if (!range) return fail(p, VX_ERR_CUDA, "libcuda.so.1 / cuMemGetAddressRange_v2 not found");
+    unsigned long long base = 0;
+    size_t size = 0;
+    if (range(&base, &size, (unsigned long long)(uintptr_t)p->ws) != 0)
+        return fail(p, VX_ERR_CUDA, "cuMemGetAddressRange failed for the workspace");
+    cudaIpcMemHandle_t h;
+    cudaError_t e = cudaIpcGetMemHandle(&h, (void *)(uintptr_t)base);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaIpcGetMemHandle");
+    memcpy(handle, &h, 64);
+    *offset = (uint64_t)((uintptr_t)p->ws - (uintptr_t)base);
+    return VX_OK;
+}
+
+vx_status vx_ipc_open(const uint8_t handle[64], uint64_t offset, void **dev_mapped_base, void **dev_workspace)
+{
+    if (!handle || !dev_mapped_base || !dev_workspace) return VX_ERR_ARG;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    void *base = NULL;
+    if (cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        cudaGetLastError();
+        return VX_ERR_CUDA;
+    }
+    *dev_mapped_base = base;
+    *dev_workspace = (uint8_t *)base + offset;
+    return VX_OK;
+}
+
+vx_status vx_ipc_close(void *dev_mapped_base)
+{
+    if (!dev_mapped_base) return VX_ERR_ARG;
+    return cudaIpcCloseMemHandle(dev_mapped_base) == cudaSuccess ? VX_OK : VX_ERR_CUDA;
 }
 
 vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64_t **dev_t1_offsets,

@@ -99,3 +99,72 @@ def test_shard_arguments(vx):
     assert vx.shard_owner(31, 24, 8, 3) == (3 << 28, 4 << 28, 3 << 21, 4 << 21)
     with pytest.raises(vx.VxError):
         vx.shard_owner(31, 24, 3, 0)                         # world must be a power of two
+
+
+# ------------------------------------------------------------------ the ranks as separate processes
+# Two processes on the ONE GPU of this box, each with its own plot and workspace; the workspaces are mapped
+# into each other with CUDA IPC (vx_ipc_export / vx_ipc_open), the barriers are torch.distributed's (gloo:
+# NCCL does not take two ranks on one device).  This is the multi-process path of a multi-GPU node
+# (paper_2606_14007_b200.ShardedPlot) with the two "GPUs" being one; the kernels never wait on one another.
+def _ipc_worker(rank, world, port, K, B, seed, out):
+    import os
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    sys.path.insert(0, os.path.join(root, "tests"))
+    import torch
+    import torch.distributed as dist
+    import paper_2606_14007_b200 as vxm
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        key = vx_inputs.key_from_seed(seed)
+        sp = vxm.ShardedPlot(K, key, rank, world, "cuda:0", bucket_bits=B)
+        for _ in range(2):                                   # twice: the second build reuses everything
+            sp.build_table1()
+            sp.plot.sort_match_table2()
+        off1, raw1 = sp.plot.read_tables(1)
+        off2, raw2 = sp.plot.read_tables(2)
+        st = sp.plot.get_stats()
+        b0, b1 = sp.plot.pass_buckets()
+        sp.close()
+        out.put((rank, b0, b1, off1, raw1, off2, raw2, st))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+@pytest.mark.parametrize("K,B,seed", [(18, 12, 9), (22, 24, 22)])
+def test_sharded_build_two_processes_cuda_ipc(vx, K, B, seed):
+    import socket
+    import torch.multiprocessing as mp
+    world = 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_ipc_worker, args=(r, world, port, K, B, seed, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted([out.get(timeout=240) for _ in range(world)], key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
+    t1 = t2 = 0
+    for rank, b0, b1, off1, raw1, off2, raw2, st in res:
+        assert (b0, b1) == (rank << (B - 1), (rank + 1) << (B - 1))
+        lo, hi = int(o_off[b0]), int(o_off[b1])
+        assert np.array_equal(off1, o_off[b0:b1 + 1] - o_off[b0])
+        assert np.array_equal(raw1, oracle.serialize_t1(4, o_non[lo:hi], o_has[lo:hi]))
+        l2, h2 = int(o_t2o[b0]), int(o_t2o[b1])
+        assert np.array_equal(off2, o_t2o[b0:b1 + 1] - o_t2o[b0])
+        g1, g2 = canon_t2(off2, *decode_t2(raw2, 4))
+        assert np.array_equal(g1, o_n1[l2:h2]) and np.array_equal(g2, o_n2[l2:h2])
+        t1 += st["t1_records"]
+        t2 += st["t2_records"]
+    assert t1 == 1 << K and t2 == len(o_n1)
