@@ -564,6 +564,85 @@ def run_probe_alu(args):
     return 0
 
 
+def run_one_plot(args):
+    """--one-plot: ONE plot over the N ranks instead of one plot per rank: rank r hashes
+    its nonce share, the records cross to their owners inside stage 1 (peer stores over NVLink), every rank
+    sorts and matches its bucket range.  "scaling": "strong".  Ranks that must share a device (a one-GPU
+    box) run over gloo: a functional check, not a measurement."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_2606_14007_b200 as vx
+    import vx_inputs
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world < 2:
+        raise SystemExit("bench.py --one-plot needs --gpus 2, 4 or 8 (torch.distributed.run)")
+    shared = torch.cuda.device_count() < int(os.environ.get("LOCAL_WORLD_SIZE", str(world)))
+    dev = torch.device("cuda", 0 if shared else local)
+    torch.cuda.set_device(dev)
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    dist.init_process_group("gloo" if shared else "nccl", **({} if shared else {"device_id": dev}))
+    K = args.K
+    key = vx_inputs.config_key(K)
+    sp = vx.ShardedPlot(K, key, rank, world, dev, bucket_bits=BUCKET_BITS)
+    stream = torch.cuda.current_stream()
+
+    def step(evs=None):
+        if evs: evs[0].record(stream)
+        sp.build_table1(stream)
+        if evs: evs[1].record(stream)
+        sp.plot.sort_match_table2(stream)
+        if evs: evs[2].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        dist.barrier()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    stats = sp.plot.get_stats()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(dev.index)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    sampler.mark()
+    for i in range(args.steps):
+        step(evs[i])
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = evs[0][0].elapsed_time(evs[-1][2])
+    s1 = statistics.mean(e[0].elapsed_time(e[1]) for e in evs)
+    s2 = statistics.mean(e[1].elapsed_time(e[2]) for e in evs)
+    t = torch.tensor([total_ms, s1, s2], dtype=torch.float64, device=None if shared else dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    cnt = torch.tensor([stats["t1_records"], stats["t2_records"]], dtype=torch.int64, device=None if shared else dev)
+    dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    total_ms, s1, s2 = (float(x) for x in t.tolist())
+    if rank == 0:
+        ms = total_ms / args.steps
+        cfg = make_config(K)
+        cfg["plots_per_gpu"] = f"1/{world} (one plot over {world} ranks)"
+        cfg["parallelism"] = (f"nonce range split {world} ways, buckets owned by hash range, all-to-all fused with "
+                              "stage 1 (peer stores + peer atomics), bucket-local sort + match")
+        line = {"metric": METRIC, "value": (1 << K) / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "u32/u64", "data": "synthetic", "config": cfg,
+                "stages": {"build_table1_sharded": {"ms": s1}, "sort_match_table2": {"ms": s2}},
+                "table_stats": {"t1_records": int(cnt[0]), "t2_records": int(cnt[1])},
+                "ranks_share_one_device": shared,
+                "note": ("functional run: the ranks share one GPU, gloo barriers" if shared else
+                         "device time per rank between CUDA events, max over ranks; host barriers inside the step"),
+                "gpu_launches": 5 * args.steps, "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    sp.close()
+    dist.destroy_process_group()
+    return 0
+
+
 def run_farm(vx, torch, K, key, dev, plot, rec_a, off_a, rec_cap, nb, slices, steps_each):
     """Two host threads, each plotting end to end into its own workspace and pinned buffers:
     whole-plot throughput with the PCIe egress of one plot hidden behind the kernels of the other."""
@@ -617,6 +696,8 @@ def main():
                     help="cpu_baseline: the oracle makes this plot in full (hashing on nproc threads), and K=20 on one")
     ap.add_argument("--flags", type=int, default=0,
                     help="test-only layout flags (1 wide layout, 2 big tiles): ncu captures of the K>=32 geometries at small K")
+    ap.add_argument("--one-plot", dest="one_plot", action="store_true",
+                    help="with --gpus N > 1: ONE plot sharded over the N ranks (strong scaling) instead of one plot per rank")
     ap.add_argument("--probe-alu", dest="probe_alu", action="store_true",
                     help="integer-pipe issue rates from dependent-free instruction chains (vx_probe_alu), one JSON line")
     ap.add_argument("--ref-K", dest="ref_K", type=int, default=22, help="oracle sample size per --impl reference step")
@@ -642,6 +723,8 @@ def main():
             cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
                    "--master-addr", "127.0.0.1", "--master-port", "29541", os.path.abspath(__file__)] + sys.argv[1:]
             return subprocess.call(cmd)
+    if args.one_plot:
+        return run_one_plot(args)
     return run_cuda(args)
 
 
