@@ -744,7 +744,9 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     const bool big = g.tile_log == VX_TILE_LOG_BIG;
     uint64_t grid = (uint64_t)num_sms * (big ? 1 : VX_S2_MINB);
 #ifdef VX_EXP_GRID_PER_SM
-    grid = (uint64_t)num_sms * VX_EXP_GRID_PER_SM;      // experiment: CTAs per SM
+    // measurement only (DESIGN.md 6.2 "what bounds it"): VX_NVCC_EXTRA=-DVX_EXP_GRID_PER_SM=1 runs the fused
+    // kernel with one resident tile per SM; never defined in the product build
+    grid = (uint64_t)num_sms * VX_EXP_GRID_PER_SM;
 #endif
     if (grid > tile_end - tile_begin) grid = tile_end - tile_begin;
     if (big && g.wide) VX_S2B_KERNEL(true)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
