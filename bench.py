@@ -465,7 +465,7 @@ def run_cuda(args):
 
     # ---- Table-2 re-keying, outside the step: one more stage a plot file needs ---------
     rekey_ms = None
-    if rank == 0 and passes == 1 and not plot.wide:
+    if rank == 0 and passes == 1:
         plot.build_table1(stream)
         plot.sort_match_table2(stream)
         r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

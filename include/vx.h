@@ -148,8 +148,11 @@ vx_status vx_sort_match_table2_to_file(vx_plot *p, void *compute_stream, void *c
  *                     the pairs by H2 >> (64 - B), each bucket in H2 order, with CSR offsets.  The
  *                     {H2, pair index} records are built in Table 1's partition array: TABLE 1 IS GONE
  *                     afterwards (vx_read_tables(1) / vx_device_tables return VX_ERR_STATE), Table 2
- *                     itself stays readable.  Enqueues only.  One-pass plots with 4-byte nonces
- *                     (K <= 32); otherwise VX_ERR_UNSUPPORTED.
+ *                     itself stays readable.  Enqueues only.  One-pass plots (K <= 33; with 5-byte
+ *                     nonces the 10 message bytes are three BLAKE3 message words and the records are
+ *                     kept in the wide 10-byte layout, a = (H2 << pb) | (index >> 16), b = index &
+ *                     0xffff); a plot made in passes returns VX_ERR_UNSUPPORTED (the pair hash scatters
+ *                     over all buckets: every pair must be resident).
  *   vx_read_tables(p, VX_TABLE2_REKEYED, ...)  the re-keyed buckets in the external Table-2 record
  *                     format (the order of pairs with equal H2 is unspecified, reading A20).
  *   vx_write_plot_file  header "VXPLOT\0\1" | u32 K | u32 B | u32 NONCE_SIZE | u32 0 | key[32] |

@@ -491,8 +491,8 @@ vx_status vx_rekey_table2(vx_plot *p, void *cuda_stream)
     if (!p) return VX_ERR_ARG;
     if (p->state < VX_MATCHED) return fail(p, VX_ERR_STATE, "vx_rekey_table2 before vx_sort_match_table2");
     if (p->state >= VX_REKEYED) return fail(p, VX_ERR_STATE, "Table 2 is already re-keyed");
-    if (p->g.wide || p->g.passes_log)
-        return fail(p, VX_ERR_UNSUPPORTED, "re-keying is implemented for one-pass plots in the 16-byte record layout (K <= 32)");
+    if (p->g.passes_log)
+        return fail(p, VX_ERR_UNSUPPORTED, "re-keying needs the whole of Table 2 resident: one-pass plots only (K <= 33)");
     p->stream = (cudaStream_t)cuda_stream;
     cudaError_t e = vx_launch_rekey(p->g, p->hc2, p->ws, p->stream);
     if (e == cudaSuccess) e = vx_launch_stage2(p->g, p->ws, false, p->force_exact, p->num_sms, p->stream);

@@ -61,25 +61,26 @@ struct VxSchedule {
     }
 };
 
+// (m2 is the compile-time constant 0 everywhere except in the 10-byte pair hash of the re-keying)
 template <int R, int SLOT>
-__device__ __forceinline__ uint32_t vx_msg(uint32_t m0, uint32_t m1)
+__device__ __forceinline__ uint32_t vx_msg(uint32_t m0, uint32_t m1, uint32_t m2)
 {
     constexpr VxSchedule S{};
     constexpr int w = S.idx[R][SLOT];
-    return w == 0 ? m0 : (w == 1 ? m1 : 0u);
+    return w == 0 ? m0 : (w == 1 ? m1 : (w == 2 ? m2 : 0u));
 }
 
 template <int R>
-__device__ __forceinline__ void vx_round(uint32_t (&v)[16], uint32_t m0, uint32_t m1)
+__device__ __forceinline__ void vx_round(uint32_t (&v)[16], uint32_t m0, uint32_t m1, uint32_t m2 = 0u)
 {
-    VX_G(v[0], v[4], v[8], v[12], (vx_msg<R, 0>(m0, m1)), (vx_msg<R, 1>(m0, m1)));
-    VX_G(v[1], v[5], v[9], v[13], (vx_msg<R, 2>(m0, m1)), (vx_msg<R, 3>(m0, m1)));
-    VX_G(v[2], v[6], v[10], v[14], (vx_msg<R, 4>(m0, m1)), (vx_msg<R, 5>(m0, m1)));
-    VX_G(v[3], v[7], v[11], v[15], (vx_msg<R, 6>(m0, m1)), (vx_msg<R, 7>(m0, m1)));
-    VX_G(v[0], v[5], v[10], v[15], (vx_msg<R, 8>(m0, m1)), (vx_msg<R, 9>(m0, m1)));
-    VX_G(v[1], v[6], v[11], v[12], (vx_msg<R, 10>(m0, m1)), (vx_msg<R, 11>(m0, m1)));
-    VX_G(v[2], v[7], v[8], v[13], (vx_msg<R, 12>(m0, m1)), (vx_msg<R, 13>(m0, m1)));
-    VX_G(v[3], v[4], v[9], v[14], (vx_msg<R, 14>(m0, m1)), (vx_msg<R, 15>(m0, m1)));
+    VX_G(v[0], v[4], v[8], v[12], (vx_msg<R, 0>(m0, m1, m2)), (vx_msg<R, 1>(m0, m1, m2)));
+    VX_G(v[1], v[5], v[9], v[13], (vx_msg<R, 2>(m0, m1, m2)), (vx_msg<R, 3>(m0, m1, m2)));
+    VX_G(v[2], v[6], v[10], v[14], (vx_msg<R, 4>(m0, m1, m2)), (vx_msg<R, 5>(m0, m1, m2)));
+    VX_G(v[3], v[7], v[11], v[15], (vx_msg<R, 6>(m0, m1, m2)), (vx_msg<R, 7>(m0, m1, m2)));
+    VX_G(v[0], v[5], v[10], v[15], (vx_msg<R, 8>(m0, m1, m2)), (vx_msg<R, 9>(m0, m1, m2)));
+    VX_G(v[1], v[6], v[11], v[12], (vx_msg<R, 10>(m0, m1, m2)), (vx_msg<R, 11>(m0, m1, m2)));
+    VX_G(v[2], v[7], v[8], v[13], (vx_msg<R, 12>(m0, m1, m2)), (vx_msg<R, 13>(m0, m1, m2)));
+    VX_G(v[3], v[4], v[9], v[14], (vx_msg<R, 14>(m0, m1, m2)), (vx_msg<R, 15>(m0, m1, m2)));
 }
 
 // H(n) as the big-endian u64 of the first 8 digest bytes (readings A4, A5).
@@ -115,6 +116,39 @@ __device__ __forceinline__ uint64_t vx_blake3_h(const VxHashConst &hc, uint32_t 
     vx_round<6>(v, m0, m1);
     const uint32_t w0 = v[0] ^ v[8], w1 = v[1] ^ v[9];
     // digest bytes 0..7 = w0, w1 little-endian; H reads them big-endian
+    return ((uint64_t)__byte_perm(w0, 0, 0x0123) << 32) | (uint64_t)__byte_perm(w1, 0, 0x0123);
+}
+
+// H2 of a pair of 5-byte nonces (re-keying, reading A19): the 10 message bytes nonce1 LE || nonce2 LE are
+// the words m0, m1, m2; column 1 of round 1 then depends on the message (m2) and is computed here from
+// the key instead of being taken from the host fold; columns 2 and 3 are the folded ones (hc.block_len = 10).
+__device__ __forceinline__ uint64_t vx_blake3_h3(const VxHashConst &hc, uint32_t m0, uint32_t m1, uint32_t m2)
+{
+    uint32_t v[16];
+    v[0] = hc.s04 + m0;
+    v[12] = vx_rotr(v[0], 16);
+    v[8] = VX_IV0 + v[12];
+    v[4] = vx_rotr(hc.k[4] ^ v[8], 12);
+    v[0] = v[0] + v[4] + m1;
+    v[12] = vx_rotr(v[12] ^ v[0], 8);
+    v[8] = v[8] + v[12];
+    v[4] = vx_rotr(v[4] ^ v[8], 7);
+    // column 1: G(v1, v5, v9, v13, m2, 0) with v1 = k1, v5 = k5, v9 = IV1, v13 = counter high = 0
+    v[1] = hc.k[1]; v[5] = hc.k[5]; v[9] = VX_IV1; v[13] = 0u;
+    VX_G(v[1], v[5], v[9], v[13], m2, 0u);
+    v[2] = hc.col[4]; v[6] = hc.col[5]; v[10] = hc.col[6]; v[14] = hc.col[7];
+    v[3] = hc.col[8]; v[7] = hc.col[9]; v[11] = hc.col[10]; v[15] = hc.col[11];
+    VX_G(v[0], v[5], v[10], v[15], 0u, 0u);
+    VX_G(v[1], v[6], v[11], v[12], 0u, 0u);
+    VX_G(v[2], v[7], v[8], v[13], 0u, 0u);
+    VX_G(v[3], v[4], v[9], v[14], 0u, 0u);
+    vx_round<1>(v, m0, m1, m2);
+    vx_round<2>(v, m0, m1, m2);
+    vx_round<3>(v, m0, m1, m2);
+    vx_round<4>(v, m0, m1, m2);
+    vx_round<5>(v, m0, m1, m2);
+    vx_round<6>(v, m0, m1, m2);
+    const uint32_t w0 = v[0] ^ v[8], w1 = v[1] ^ v[9];
     return ((uint64_t)__byte_perm(w0, 0, 0x0123) << 32) | (uint64_t)__byte_perm(w1, 0, 0x0123);
 }
 

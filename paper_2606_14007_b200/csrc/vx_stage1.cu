@@ -405,9 +405,61 @@ __global__ void vx_k_save_t1_total(const unsigned long long *__restrict__ part_b
     ctrl->t1_total = part_base[P];
 }
 
+// The same in the wide layout (K >= 33, or forced): Table 2 is resident packed (uint2 {n1 lo, n2 lo} + a
+// byte of high bits) and the partition array holds 10-byte records -- a = (H2 << pb) | (index >> 16),
+// b = index & 0xffff: the pb bits the prefix frees hold the high bits of the 33-bit pair index, exactly as
+// they hold the high nonce bits in Table 1, so the wide sort kernel orders (a, b) = (H2, index) unchanged.
+// Two scattered stores per record (the scratch of stage 1's rounds aliases the Table-2 region, which is
+// live here): 1.8x the one-store kernel, off the plot path.
+template <bool NONCE5>
+__global__ void __launch_bounds__(VX_S1_THREADS)
+vx_k_rekey_scatter_wide(const __grid_constant__ VxHashConst hc2, const uint2 *__restrict__ t2_rec,
+                        const uint8_t *__restrict__ t2_hi, uint32_t pb, uint32_t cap, uint32_t cap_check,
+                        unsigned long long *__restrict__ part_a, uint16_t *__restrict__ part_b,
+                        uint32_t *__restrict__ cursor, VxCtrl *__restrict__ ctrl)
+{
+    const unsigned long long M = ctrl->t2_total;
+    const uint64_t base = (uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) + threadIdx.x;
+    if ((uint64_t)blockIdx.x * (VX_S1_THREADS * VX_S1_NPT) >= M) return;
+    if (pb + 16 < 64 && (M >> (pb + 16)) != 0) {        // the pair index must fit pb + 16 bits
+        if (base == 0) atomicOr(&ctrl->flags, VX_FLAG_T2_OVERFLOW);
+        return;
+    }
+    uint64_t H[VX_S1_NPT];
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t r = base + (uint64_t)k * VX_S1_THREADS;
+        const uint2 pr = r < M ? __ldcs(t2_rec + r) : make_uint2(0u, 0u);
+        if constexpr (NONCE5) {
+            const uint32_t hb = r < M ? t2_hi[r] : 0u;  // (n1 >> 32) | (n2 >> 32) << 4
+            // message bytes: n1[0..4] n2[0..4]
+            const uint32_t m1 = (hb & 15u) | (pr.y << 8);
+            const uint32_t m2 = (pr.y >> 24) | ((hb >> 4) << 8);
+            H[k] = vx_blake3_h3(hc2, pr.x, m1, m2);
+        } else {
+            H[k] = vx_blake3_h<true>(hc2, pr.x, pr.y);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < VX_S1_NPT; k++) {
+        const uint64_t r = base + (uint64_t)k * VX_S1_THREADS;
+        if (r < M) {
+            const uint32_t p = pb ? (uint32_t)(H[k] >> (64 - pb)) : 0u;
+            const uint32_t slot = atomicAdd(&cursor[p], 1u);
+            if (slot < cap_check) {
+                const size_t at = (size_t)p * cap + slot;
+                part_a[at] = (pb ? H[k] << pb : H[k]) | (r >> 16);
+                part_b[at] = (uint16_t)(r & 0xffffu);
+            } else {
+                atomicOr(&ctrl->flags, VX_FLAG_PART_OVERFLOW);
+            }
+        }
+    }
+}
+
 cudaError_t vx_launch_rekey(const VxGeom &g, const VxHashConst &hc2, uint8_t *ws, cudaStream_t st)
 {
-    if (g.wide || g.passes_log) return cudaErrorInvalidValue;
+    if (g.passes_log) return cudaErrorInvalidValue;
     VxCtrl *ctrl = (VxCtrl *)(ws + g.off_ctrl);
     uint32_t *cursor = (uint32_t *)(ws + g.off_cursor);
     vx_k_save_t1_total<<<1, 1, 0, st>>>((const unsigned long long *)(ws + g.off_part_base), g.P, ctrl);
@@ -416,8 +468,19 @@ cudaError_t vx_launch_rekey(const VxGeom &g, const VxHashConst &hc2, uint8_t *ws
     if (e != cudaSuccess) return e;
     const uint64_t per_cta = (uint64_t)VX_S1_THREADS * VX_S1_NPT;
     const uint64_t grid = (g.t2_cap + per_cta - 1) / per_cta;          // upper bound; CTAs beyond |Table 2| exit
-    vx_k_rekey_scatter<<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc2, (const uint2 *)(ws + g.off_t2_rec), g.pb, g.cap,
-                                                                 g.cap_check, (uint4 *)(ws + g.off_part), cursor, ctrl);
+    if (g.wide) {
+        unsigned long long *part_a = (unsigned long long *)(ws + g.off_part);
+        uint16_t *part_b = (uint16_t *)(ws + g.off_part_b);
+        if (g.nonce_size == 5)
+            vx_k_rekey_scatter_wide<true><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
+                hc2, (const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi, g.pb, g.cap, g.cap_check, part_a, part_b, cursor, ctrl);
+        else
+            vx_k_rekey_scatter_wide<false><<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(
+                hc2, (const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi, g.pb, g.cap, g.cap_check, part_a, part_b, cursor, ctrl);
+    } else {
+        vx_k_rekey_scatter<<<(unsigned)grid, VX_S1_THREADS, 0, st>>>(hc2, (const uint2 *)(ws + g.off_t2_rec), g.pb, g.cap,
+                                                                     g.cap_check, (uint4 *)(ws + g.off_part), cursor, ctrl);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     vx_k_partition_scan<<<1, VX_SCAN_THREADS, 0, st>>>(cursor, g.cap_check, g.P,

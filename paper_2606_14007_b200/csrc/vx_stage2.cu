@@ -626,13 +626,57 @@ vx_k_export_rekey(const uint4 *__restrict__ part, const unsigned long long *__re
     }
 }
 
+// the same in the wide layout: pair index = (low pb bits of a) << 16 | b; the pair comes from the packed
+// Table 2 and leaves in the external format, nonce1[NS] || nonce2[NS]
+template <int NS>
+__global__ void __launch_bounds__(256)
+vx_k_export_rekey_wide(const unsigned long long *__restrict__ part_a, const uint16_t *__restrict__ part_b,
+                       const unsigned long long *__restrict__ part_base, uint32_t P, uint32_t cap, uint32_t pb,
+                       const uint2 *__restrict__ t2_rec, const uint8_t *__restrict__ t2_hi,
+                       unsigned long long first, unsigned long long count, uint8_t *__restrict__ out)
+{
+    for (unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; r < count;
+         r += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long g = first + r;
+        uint32_t lo = 0, hi = P;
+        while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (part_base[mid] <= g) lo = mid; else hi = mid;
+        }
+        const size_t slot = (size_t)lo * cap + (g - part_base[lo]);
+        const unsigned long long idx = ((part_a[slot] & ((1ull << pb) - 1ull)) << 16) | part_b[slot];
+        const uint2 v = t2_rec[idx];
+        if constexpr (NS == 4) {
+            reinterpret_cast<uint2 *>(out)[r] = v;
+        } else {
+            const uint8_t h = t2_hi[idx];
+            uint8_t *o = out + 10 * r;
+#pragma unroll
+            for (int j = 0; j < 4; j++) { o[j] = (uint8_t)(v.x >> (8 * j)); o[5 + j] = (uint8_t)(v.y >> (8 * j)); }
+            o[4] = h & 15u;
+            o[9] = h >> 4;
+        }
+    }
+}
+
 cudaError_t vx_launch_export_rekey(const VxGeom &g, uint8_t *ws, uint64_t first, uint64_t count, cudaStream_t st)
 {
     if (count == 0) return cudaSuccess;
     uint64_t grid = (count + 255) / 256;
     if (grid > (uint64_t)vx_sm_count() * 16) grid = (uint64_t)vx_sm_count() * 16;
-    vx_k_export_rekey<<<(unsigned)grid, 256, 0, st>>>((const uint4 *)(ws + g.off_part),
-                                                      (const unsigned long long *)(ws + g.off_part_base), (uint32_t)g.P,
+    const unsigned long long *pbase = (const unsigned long long *)(ws + g.off_part_base);
+    if (g.wide) {
+        const unsigned long long *pa = (const unsigned long long *)(ws + g.off_part);
+        const uint16_t *pbb = (const uint16_t *)(ws + g.off_part_b);
+        if (g.nonce_size == 5)
+            vx_k_export_rekey_wide<5><<<(unsigned)grid, 256, 0, st>>>(pa, pbb, pbase, (uint32_t)g.P, g.cap, g.pb,
+                (const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi, first, count, ws + g.off_stage);
+        else
+            vx_k_export_rekey_wide<4><<<(unsigned)grid, 256, 0, st>>>(pa, pbb, pbase, (uint32_t)g.P, g.cap, g.pb,
+                (const uint2 *)(ws + g.off_t2_rec), ws + g.off_t2_hi, first, count, ws + g.off_stage);
+        return cudaGetLastError();
+    }
+    vx_k_export_rekey<<<(unsigned)grid, 256, 0, st>>>((const uint4 *)(ws + g.off_part), pbase, (uint32_t)g.P,
                                                       g.cap, (const uint2 *)(ws + g.off_t2_rec), first, count,
                                                       (uint2 *)(ws + g.off_stage));
     return cudaGetLastError();

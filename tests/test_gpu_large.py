@@ -490,6 +490,80 @@ def test_K33_full_size_samples_and_properties(vx):
     plot.free()
 
 
+def test_K33_rekeyed_table2(vx):
+    """SURVEY 8(f2) at BASELINE.json configs[4]: 2^33 pairs of 5-byte nonces re-keyed by the hash of their
+    10 bytes (three message words) in the wide layout.  Sampled buckets: every record's pair hash from the
+    oracle, bucket = its prefix, H2 non-decreasing, the pair present in Table 2's source bucket; whole
+    table on the device: CSR offsets consistent and every pair index exactly once."""
+    import torch
+    K, B = 33, 24
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    need = vx.workspace_bytes(K)
+    if free < need + (6 << 30):
+        pytest.skip(f"needs {need / 1e9:.0f} GB + 6 GB of device memory, {free / 1e9:.0f} GB free")
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    plot.sort_match_table2()
+    st = plot.get_stats()
+    M = st["t2_records"]
+    a, b, pb, o1, o2 = wide_views(plot)                  # views of the workspace: they show the re-keyed records below
+    plot.rekey_table2()
+    st2 = plot.get_stats()
+    assert st2["t1_records"] == 1 << K and st2["t2_records"] == M
+    rng = np.random.default_rng(133)
+    NB = 1 << B
+    checked = 0
+    for b0 in [0, NB - 4] + [int(x) for x in rng.integers(0, NB - 4, 10)]:
+        off, raw = plot.read_tables(vx.VX_TABLE2_REKEYED, b0, b0 + 4)
+        n1, n2 = decode_t2(raw, 5)
+        h = np.array([oracle.hash_pair(key, int(a), int(b), 5) for a, b in zip(n1, n2)], dtype=np.uint64)
+        ids = np.repeat(np.arange(b0, b0 + 4, dtype=np.uint64), np.diff(off).astype(np.int64))
+        assert np.array_equal(h >> np.uint64(64 - B), ids), "a pair sits in a bucket that is not its H2 prefix"
+        assert bool(np.all(np.diff(h.astype(np.int64) ^ SIGN) >= 0)), "re-keyed buckets are not in H2 order"
+        # each sampled pair is a match of Table 2: same source bucket, hashes within T, ordered
+        h1 = np.array([oracle.hash_nonce(key, int(a), 5) for a in n1[:64]], dtype=np.uint64)
+        h2 = np.array([oracle.hash_nonce(key, int(b), 5) for b in n2[:64]], dtype=np.uint64)
+        assert bool(np.all(h1 >> np.uint64(64 - B) == h2 >> np.uint64(64 - B)))
+        d = h2 - h1
+        assert bool(np.all(h2 >= h1)) and bool(np.all(d < np.uint64(1 << (64 - K))))
+        checked += len(n1)
+    assert checked > 20000
+    # whole table: offsets and the permutation of pair indices
+    dev = plot.device
+    pbits, cap = plot.partition_bits, plot.partition_capacity
+    P = 1 << pbits
+    cnt = pb[1:] - pb[:-1]
+    assert int(pb[0]) == 0 and int(pb[-1]) == M and int(cnt.max()) <= cap
+    assert int(o1[0]) == 0 and int(o1[-1]) == M and bool((o1[1:] >= o1[:-1]).all())
+    lane = torch.arange(cap, device=dev)[None, :]
+    chunk = (1 << 25) // cap
+    lowmask = (1 << pbits) - 1
+    R = 1 << 30
+    for r0 in range(0, M, R):
+        n_r = min(R, M - r0)
+        seen = torch.zeros(n_r, dtype=torch.bool, device=dev)
+        met = 0
+        for p0 in range(0, P, chunk):
+            ak = a[p0:p0 + chunk]
+            valid = lane < cnt[p0:p0 + chunk, None]
+            idx = ((ak & lowmask) << 16) | (b[p0:p0 + chunk].long() & 0xffff)
+            if r0 == 0:
+                k = ak ^ SIGN
+                ok = k[:, 1:] >= k[:, :-1]
+                assert bool((ok | ~valid[:, 1:]).all()), "a partition is not in H2 order"
+                assert bool((idx[valid] < M).all())
+                del k, ok
+            sel = valid & (idx >= r0) & (idx < r0 + n_r)
+            seen[idx[sel] - r0] = True
+            met += int(sel.sum())
+            del ak, valid, idx, sel
+        assert met == n_r and int(seen.sum()) == n_r, "a pair is missing from the re-keyed table (or appears twice)"
+        del seen
+    plot.free()
+
+
 def test_K34_two_bucket_range_passes(vx):
     """K = 34: 2^34 nonces in two bucket-range passes, each the size of
     a K = 33 plot and checked like one; over the two passes every nonce is met exactly once."""

@@ -27,7 +27,7 @@ def canon_rekeyed(off, n1, n2, h2):
     return n1[order], n2[order], h2[order]
 
 
-@pytest.mark.parametrize("big", [0, 2])
+@pytest.mark.parametrize("big", [0, 2, 1, 3])      # narrow / big tiles / wide / big + wide (vx.VX_CREATE_* flags)
 @pytest.mark.parametrize("K,B,seed", [(10, 6, 2), (12, 8, 1), (14, 9, 5), (16, 12, 1), (16, 7, 6), (18, 24, 3),
                                       (20, 24, 1), (21, 12, 2), (22, 24, 22)])
 def test_rekeyed_table2_and_plot_file_vs_oracle(vx, K, B, seed, big):
@@ -101,7 +101,7 @@ def test_rekeyed_table2_and_plot_file_vs_oracle(vx, K, B, seed, big):
 def test_rekey_unsupported_layouts_and_errors(vx):
     import torch
     key = vx_inputs.key_from_seed(1)
-    for flags in (vx.VX_CREATE_WIDE_LAYOUT, vx.VX_CREATE_PASSES_LOG(1)):
+    for flags in (vx.VX_CREATE_PASSES_LOG(1), vx.VX_CREATE_PASSES_LOG(1) | vx.VX_CREATE_WIDE_LAYOUT):
         p = vx.Plot(16, key, 12, flags=flags)
         p.build_table1()
         p.sort_match_table2()
