@@ -176,7 +176,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     uint32_t *E = bins + VX_NBINS + 32;                 // CAPA + 1 (+ pad): match-count prefix
     uint32_t *sub = E;                                  // phases C-D only: 32-bit ranking sub-keys
     __shared__ uint32_t s_warp[32];
-    __shared__ uint32_t s_tile, s_tie;
+    __shared__ uint32_t s_tile, s_tie, s_cnt;
     __shared__ unsigned long long s_base2;
     // deferred emit (phase H of tile t runs after phase A of the CTA's next tile): Table-2 prefix at
     // the first record of every bucket of tile t, saved before the bins are recycled
@@ -258,6 +258,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         if (tid == 0) {
             const uint32_t t = q.tile_begin + atomicAdd(&q.ctrl->ticket, 1u);
             s_tile = t;
+            // the tile's record count travels with the ticket: one thread's load behind the atomic instead of
+            // every thread's load behind the barrier
+            s_cnt = t < q.tile_end ? min(q.cursor[t], q.cap_check) : 0u;
             // Tickets are handed out in partition order and the CTAs run about one tile apart, so the
             // partition gridDim tickets ahead is the one some CTA (most likely this one) takes next:
             // one bulk prefetch (TMA, cp.async.bulk.prefetch.L2 -> UBLKPF.L2) brings its 64 KB into
@@ -293,7 +296,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             if (tid == 0) s_tie = 0u;                   // set in phase E, read after the sync behind it
             tile = s_tile;
             const bool valid = tile < q.tile_end;
-            cnt = valid ? min(q.cursor[tile], q.cap_check) : 0u;
+            cnt = s_cnt;
             if constexpr (WIDE) {
                 src = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned long long *>(q.part) + (size_t)tile * q.cap);
                 src_b = q.part_b + (size_t)tile * q.cap;
