@@ -428,45 +428,86 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 // guarded: lim can reach the sentinel value ~0 (narrow: only in the last tile; wide:
                 // only if the tile's largest key is ~0 itself, else lim is clamped below it)
                 const bool guarded = WIDE ? keyS[last] == ~0ull : tile == q.P - 1;
+                // three items at a time, the loads of each search step issued together (the same loads
+                // as one item after the other, but three dependency chains in flight per warp)
+                constexpr int VX_EB = 3;
+                static_assert(ITEMS % VX_EB == 0, "ITEMS must be a multiple of the phase-E batch");
 #pragma unroll
-                for (int it = 0; it < ITEMS; it++) {
-                    const uint32_t i = it * THREADS + tid;
-                    uint32_t c = 0;
-                    if (it * THREADS + wbase < cnt) {
-                        const uint64_t ki = keyS[i];
-                        const uint64_t kl = WIDE ? (ki | q.lowmask) : ki;
-                        uint64_t lim = kl + Tm1;
-                        // narrow, not the last tile: key + T stays inside the next partition, no wrap
-                        if ((WIDE || guarded) && lim < kl) lim = ~0ull;
-                        lim = min(lim, ki | bmask);
-                        if (WIDE && !guarded) lim = min(lim, (uint64_t)(~0ull - 1ull));
-                        if (!guarded) {
+                for (int g = 0; g < ITEMS; g += VX_EB) {
+                    if (g * THREADS + wbase >= cnt) {   // warp-uniform: nothing of this batch is in range
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) E[(g + u) * THREADS + tid] = 0u;
+                        continue;
+                    }
+                    if (!guarded) {
+                        uint64_t ki[VX_EB], lim[VX_EB], kn[VX_EB];
+                        uint32_t pos[VX_EB];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            const uint32_t i = (g + u) * THREADS + tid;   // i + 7 < CAPA + 8: inside keyS
+                            ki[u] = keyS[i];
+                            kn[u] = keyS[i + 1];
+                        }
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            const uint32_t i = (g + u) * THREADS + tid;
+                            const uint64_t kl = WIDE ? (ki[u] | q.lowmask) : ki[u];
+                            uint64_t l = kl + Tm1;
+                            if (WIDE && l < kl) l = ~0ull;
+                            l = min(l, ki[u] | bmask);
+                            if (WIDE) l = min(l, (uint64_t)(~0ull - 1ull));
+                            lim[u] = l;
                             // the fast pass is valid iff the keys came out strictly increasing
-                            if (!exact && i < cnt && keyS[i + 1] <= ki) s_tie = 1u;
-                            // largest o in [0, 7] with key[i + o] <= lim (keys ascend; key[cnt] = ~0 > lim)
-                            uint32_t pos = i;
-                            if (keyS[pos + 4] <= lim) pos += 4;
-                            if (keyS[pos + 2] <= lim) pos += 2;
-                            if (keyS[pos + 1] <= lim) pos += 1;
-                            c = i < cnt ? pos - i : 0u;
+                            if (!exact && i < cnt && kn[u] <= ki[u]) s_tie = 1u;
+                            pos[u] = i;
+                        }
+                        // largest o in [0, 7] with key[i + o] <= lim (keys ascend; key[cnt] = ~0 > lim)
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) kn[u] = keyS[pos[u] + 4];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) if (kn[u] <= lim[u]) pos[u] += 4;
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) kn[u] = keyS[pos[u] + 2];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) if (kn[u] <= lim[u]) pos[u] += 2;
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) kn[u] = keyS[pos[u] + 1];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) if (kn[u] <= lim[u]) pos[u] += 1;
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            const uint32_t i = (g + u) * THREADS + tid;
+                            uint32_t c = i < cnt ? pos[u] - i : 0u;
                             if (__any_sync(VX_FULL, c == 7u)) {
                                 for (uint32_t j = i + 8;; j++) {
-                                    const bool m = c >= 7u && j < cnt && keyS[min(j, last)] <= lim;
+                                    const bool m = c >= 7u && j < cnt && keyS[min(j, last)] <= lim[u];
                                     c += m ? 1u : 0u;
                                     if (!__any_sync(VX_FULL, m)) break;
                                 }
                             }
-                        } else {
+                            VX_CHECK(q.ctrl, i < (uint32_t)CAPA && (c == 0 || i + c < cnt));
+                            E[i] = c;
+                        }
+                    } else {
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            const uint32_t i = (g + u) * THREADS + tid;
+                            const uint64_t ki = keyS[i];
+                            const uint64_t kl = WIDE ? (ki | q.lowmask) : ki;
+                            uint64_t lim = kl + Tm1;
+                            if (lim < kl) lim = ~0ull;
+                            lim = min(lim, ki | bmask);
+                            uint32_t c = 0;
                             if (!exact && i < last && keyS[i + 1] <= ki) s_tie = 1u;
                             for (uint32_t j = i + 1;; j++) {
-                                const bool m = j < cnt && keyS[min(j, last)] <= lim;
+                                const bool m = i < cnt && j < cnt && keyS[min(j, last)] <= lim;
                                 c += m ? 1u : 0u;
                                 if (!__any_sync(VX_FULL, m)) break;
                             }
+                            VX_CHECK(q.ctrl, i < (uint32_t)CAPA && (c == 0 || i + c < cnt));
+                            E[i] = c;
                         }
                     }
-                    VX_CHECK(q.ctrl, i < (uint32_t)CAPA && (c == 0 || i + c < cnt));
-                    E[i] = c;
                 }
             }
             __syncthreads();
