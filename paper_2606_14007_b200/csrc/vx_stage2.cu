@@ -206,7 +206,12 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     // ---- look-back for the Table-2 base, then H: the matches of i are i+1 .. i+c_i, c_i = E[i+1] - E[i]
     auto lookback_emit = [&](uint32_t tile, uint32_t cnt, uint32_t M) {
         if (tid < 32) {
+#ifdef VX_EXP_NO_LOOKBACK
+            // measurement only: no look-back, Table 2 lands at tile * 4000 -- WRONG tables, right timing
+            const unsigned long long b2 = (unsigned long long)tile * 4000ull;
+#else
             const unsigned long long b2 = vx_lookback(q.status, tile, M, lane);
+#endif
             if (tid == 0) {
                 s_base2 = b2;
                 if (tile == q.tile_end - 1 && q.slice_end_out) *q.slice_end_out = b2 + M;
