@@ -349,19 +349,24 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             __syncthreads();
             // ---- C. scatter to bin start + slot (bank-random, the only such pass) ------------------
             // sub[] = the 32 hash bits below the bin index: what the fast ranking pass compares
+            //      (all bin starts are fetched before the first store: nine independent loads in flight)
+            {
+                uint32_t pos[ITEMS];
 #pragma unroll
-            for (int it = 0; it < ITEMS; it++) {
-                if (it * THREADS + wbase < cnt) {       // warp-uniform
+                for (int it = 0; it < ITEMS; it++) {
                     const uint32_t idx = it * THREADS + tid;
-                    if (idx < cnt) {
-                        const uint32_t pos = bins[vx_bin<VX_NBINS>(key[it], sh)] + sn[it];
-                        VX_CHECK(q.ctrl, pos < cnt);
-                        keyS[pos] = key[it];
-                        nonS[pos] = non[it];
+                    pos[it] = idx < cnt ? bins[vx_bin<VX_NBINS>(key[it], sh)] + sn[it] : 0xffffffffu;
+                }
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    if (pos[it] != 0xffffffffu) {
+                        VX_CHECK(q.ctrl, pos[it] < cnt);
+                        keyS[pos[it]] = key[it];
+                        nonS[pos[it]] = non[it];
                         // ranking key: the hash bits below the bin index with the record's slot in the bin
                         // (its arrival order, unique there) in the low 4 bits -- distinct within a bin, so the
                         // ranks below are distinct and no two lanes ever write one sorted slot
-                        sub[pos] = (vx_subkey(key[it], sh) & submask) | sn[it];
+                        sub[pos[it]] = (vx_subkey(key[it], sh) & submask) | sn[it];
                         if (sn[it] > 15u) s_tie = 1u;   // a bin of more than 16 records: rank it exactly
                     }
                 }
