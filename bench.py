@@ -45,34 +45,20 @@ S1_BYTES_PER_NONCE = 12            # write the record once
 ALU_LANES_PER_SMSP = 16
 # roofline.traffic: DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per nonce of one launch
 # from an ncu --set full capture of THIS tree's kernels, per kernel geometry (layout, tile_log); the
-# bytes per nonce depend on the geometry, not on K.  Each entry names the file under profiles/ it was
-# read from; a geometry with no capture reports traffic = null rather than another geometry's number.
+# bytes per nonce depend on the geometry, not on K.  Each entry names the summary under profiles/ it was
+# read from (with the full ncu command); a geometry with no capture reports traffic = null rather than
+# another geometry's number.
 NCU_TRAFFIC = {
-    # (layout, tile_log): {"s1": B/nonce of vx_k_hash_scatter (+ vx_k_compact in the wide layout),
-    #                      "s2": B/nonce of vx_k_sort_match, "source": file}
+    # (layout, tile_log): B/nonce of stage 1 (vx_k_hash_scatter [+ vx_k_compact]) and of stage 2 (vx_k_sort_match)
+    ("narrow", 12): {"s1": 21.91, "s2": 40.31, "source": "profiles/r02_ncu.md (narrow layout, 2^12-record tiles; ncu --set full at K=29)"},
+    ("narrow", 13): {"s1": 17.18, "s2": 40.55, "source": "profiles/r02_ncu.md (narrow layout, 2^13-record tiles; ncu --set full at K=28)"},
+    ("wide", 13): {"s1": 41.22, "s2": 29.54, "source": "profiles/r02_ncu.md (wide layout, 2^13-record tiles; ncu --set full at K=28)"},
 }
 
 
 def load_ncu_traffic():
-    """profiles/r02_traffic.json: written from the round's ncu captures (see profiles/r02_ncu.md)."""
-    path = os.path.join(ROOT, "profiles", "r02_traffic.json")
-    try:
-        with open(path) as f:
-            for row in json.load(f)["geometries"]:
-                NCU_TRAFFIC[(row["layout"], int(row["tile_log"]))] = row
-    except Exception:
-        pass
-
-
-def measured_peaks():
-    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    try:
-        with open(path) as f:
-            d = json.load(f)
-        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
-                "source": "MEASURED_PEAKS.json"}
-    except Exception:
-        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
+    """(the table above is final for this tree; kept as a function so that run_cuda reads one place)"""
+    return NCU_TRAFFIC
 
 
 class ClockSampler:
