@@ -61,8 +61,10 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     vx_geom_select_pass(g, 0);
     const uint64_t mean = g->N >> g->pb;
     uint64_t cap;
-    if (g->pb == 0) cap = mean;                            // the single partition holds everything
-    else cap = mean + (uint64_t)ceil(8.0 * sqrt((double)mean));        // Poisson tail, 8 sigma
+    // Poisson tail, 8 sigma.  Also with a single partition (pb = 0), which holds exactly 2^K records in
+    // stage 1: the re-keying appends |Table 2| records to the same partitions, and |Table 2| can exceed 2^K
+    // by a few sigma when K is tiny
+    cap = mean + (uint64_t)ceil(8.0 * sqrt((double)mean));
     cap = (cap + 31) & ~(uint64_t)31;
     if (cap > (g->tile_log == VX_TILE_LOG_BIG ? VX_S2B_THREADS * VX_S2B_ITEMS : VX_S2_THREADS * VX_S2_ITEMS)) return false;
     g->cap = (uint32_t)cap;
