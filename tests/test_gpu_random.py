@@ -40,6 +40,12 @@ def test_random_geometry_vs_oracle(vx, case, K, B, flags, passes_log):
     o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_tables(K, key, B)
     plot = vx.Plot(K, key, B, flags=flags | vx.VX_CREATE_PASSES_LOG(passes_log))
     nsize = plot.nonce_size
+    opt = np.random.default_rng(77 + case)
+    if opt.integers(0, 3) == 0:
+        plot.set_option(vx.VX_OPT_FORCE_EXACT_RANK, 1)            # the exact (H, n) ranking path
+    elif opt.integers(0, 2) == 0:
+        plot.set_option(vx.VX_OPT_SUBKEY_BITS, int(opt.integers(0, 9)))   # the tie -> redo path
+    slices = int(opt.integers(1, 40))
     t1 = t2 = 0
     for s in range(plot.passes):
         if plot.passes > 1:
@@ -59,6 +65,15 @@ def test_random_geometry_vs_oracle(vx, case, K, B, flags, passes_log):
         st = plot.get_stats()
         t1 += st["t1_records"]
         t2 += st["t2_records"]
+        # the same slice again through the streamed egress, a random number of stage-2 launches
+        import torch
+        rec = torch.zeros(raw2.nbytes + 64, dtype=torch.uint8, pin_memory=True)
+        off = torch.full((b1 - b0 + 1,), -1, dtype=torch.int64, pin_memory=True)
+        plot.build_table1()
+        n = plot.sort_match_table2_to_host(torch.cuda.Stream(), rec.data_ptr(), rec.numel(), off.data_ptr(), slices=slices)
+        assert n == raw2.nbytes and np.array_equal(off.numpy().view(np.uint64), off2)
+        e1, e2 = canon_t2(off2, *decode_t2(rec.numpy()[:n], nsize))
+        assert np.array_equal(e1, g1) and np.array_equal(e2, g2)
     assert t1 == 1 << K and t2 == len(o_n1)
     if plot.passes == 1:
         plot.rekey_table2()
