@@ -490,6 +490,62 @@ def test_K33_full_size_samples_and_properties(vx):
     plot.free()
 
 
+def test_K31_rekeyed_table2(vx):
+    """SURVEY 8(f2) at BASELINE.json configs[3]: the 2.14 G pairs of the K=31 plot re-keyed by the hash of
+    the pair (16-byte {H2, pair index} records in Table 1's partition array).  Sampled buckets: every
+    record's pair hash from the oracle, bucket = its prefix, H2 non-decreasing; whole table on the device:
+    CSR offsets consistent, every partition in H2 order and inside its prefix, every pair index exactly once."""
+    import torch
+    K, B = 31, 24
+    key = vx_inputs.config_key(K)
+    plot = vx.Plot(K, key, B)
+    plot.build_table1()
+    plot.sort_match_table2()
+    M = plot.get_stats()["t2_records"]
+    part, pb, o1, o2, _ = device_views(plot)             # views of the workspace: they show the re-keyed records below
+    plot.rekey_table2()
+    st = plot.get_stats()
+    assert st["t1_records"] == 1 << K and st["t2_records"] == M
+    rng = np.random.default_rng(131)
+    NB = 1 << B
+    checked = 0
+    for b0 in [0, NB - 8] + [int(x) for x in rng.integers(0, NB - 8, 14)]:
+        off, raw = plot.read_tables(vx.VX_TABLE2_REKEYED, b0, b0 + 8)
+        n1, n2 = decode_t2(raw, 4)
+        h = np.array([oracle.hash_pair(key, int(a), int(b), 4) for a, b in zip(n1, n2)], dtype=np.uint64)
+        ids = np.repeat(np.arange(b0, b0 + 8, dtype=np.uint64), np.diff(off).astype(np.int64))
+        assert np.array_equal(h >> np.uint64(64 - B), ids), "a pair sits in a bucket that is not its H2 prefix"
+        assert bool(np.all(np.diff(h.astype(np.int64) ^ SIGN) >= 0)), "re-keyed buckets are not in H2 order"
+        checked += len(n1)
+    assert checked > 15000
+    dev = plot.device
+    pbits, cap = plot.partition_bits, plot.partition_capacity
+    P = 1 << pbits
+    cnt = pb[1:] - pb[:-1]
+    assert int(pb[0]) == 0 and int(pb[-1]) == M and int(cnt.max()) <= cap
+    assert int(o1[0]) == 0 and int(o1[-1]) == M and bool((o1[1:] >= o1[:-1]).all())
+    seen = torch.zeros(M, dtype=torch.bool, device=dev)
+    lane = torch.arange(cap, device=dev)[None, :]
+    chunk = max(1, (1 << 26) // cap)
+    for p0 in range(0, P, chunk):
+        blk = part[p0:p0 + chunk]
+        valid = lane < cnt[p0:p0 + chunk, None]
+        keyv = ((blk[..., 1].long() & 0xffffffff) << 32) | (blk[..., 0].long() & 0xffffffff)
+        idx = blk[..., 2].long() & 0xffffffff
+        pid = (keyv >> (64 - pbits)) & (P - 1)
+        want = torch.arange(p0, p0 + blk.shape[0], device=dev)[:, None].expand_as(pid)
+        assert bool((pid[valid] == want[valid]).all()), "a pair outside its partition's H2 prefix"
+        k = keyv ^ SIGN
+        ok = k[:, 1:] >= k[:, :-1]
+        assert bool((ok | ~valid[:, 1:]).all()), "a partition is not in H2 order"
+        iv = idx[valid]
+        assert bool((iv < M).all())
+        seen[iv] = True
+        del blk, valid, keyv, idx, pid, want, k, ok, iv
+    assert int(seen.sum()) == M, "a pair is missing from the re-keyed table (or appears twice)"
+    plot.free()
+
+
 def test_K33_rekeyed_table2(vx):
     """SURVEY 8(f2) at BASELINE.json configs[4]: 2^33 pairs of 5-byte nonces re-keyed by the hash of their
     10 bytes (three message words) in the wide layout.  Sampled buckets: every record's pair hash from the
