@@ -293,6 +293,17 @@ vx_status vx_hash_range(vx_plot *p, uint64_t nonce_begin, uint64_t count, uint64
 vx_status vx_hash_sink(vx_plot *p, uint64_t count, uint64_t *dev_sink, size_t sink_words,
                        void *cuda_stream);
 
+/* The same fold for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): hashes the nonces [nonce_begin, nonce_begin + count) and writes the
+ * xor of their hashes to dev_out[0] (DEVICE, one uint64).  Its scratch -- one partial word per thread
+ * block -- is a file-scope device array of libvx.so (256 KB, held by every GPU that loads the library
+ * until the process exits), so the call allocates nothing: no cudaMalloc, cudaFree or allocating library
+ * routine, and the plot need not be bound.  Limit: count <= 2^25 nonces per call, VX_ERR_RANGE beyond
+ * (text in vx_last_error).  Every call on a device shares that array: calls that overlap on the GPU
+ * (different streams or host threads) race -- serialise them on one stream.  Enqueues only. */
+vx_status vx_hash_fold_noalloc(vx_plot *p, uint64_t nonce_begin, uint64_t count, uint64_t *dev_out,
+                               void *cuda_stream);
+
 /* Measurement aid for the same roofline (the integer pipes' issue rate is not in
  * MEASURED_PEAKS.json and is to be measured with dependent-free instruction chains): launches
  * vx_sm_count x ctas_per_sm CTAs of 256 threads, each thread running 8 independent chains of

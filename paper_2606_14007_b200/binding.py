@@ -37,7 +37,7 @@ EXPORTS = ["vx_workspace_bytes", "vx_workspace_bytes_ex", "vx_workspace_bytes_op
            "vx_plot_all_passes_to_host", "vx_rekey_table2", "vx_write_plot_file", "vx_shard_owner", "vx_shard_begin", "vx_shard_scatter", "vx_shard_finish",
            "vx_ipc_export", "vx_ipc_open", "vx_ipc_close",
            "vx_device_tables", "vx_plot_set_option", "vx_get_stats", "vx_get_counters", "vx_synchronize", "vx_hash_range",
-           "vx_hash_sink", "vx_probe_alu",
+           "vx_hash_sink", "vx_probe_alu", "vx_hash_fold_noalloc",
            "vx_plot_info", "vx_plot_layout", "vx_plot_launches", "vx_last_error", "vx_status_string", "vx_free"]
 
 _u64 = ctypes.c_uint64
@@ -136,6 +136,8 @@ def load_library() -> ctypes.CDLL:
     L.vx_hash_range.argtypes = [_vp, _u64, _u64, _vp, _vp]
     L.vx_hash_sink.restype = ctypes.c_int
     L.vx_hash_sink.argtypes = [_vp, _u64, _vp, _sz, _vp]
+    L.vx_hash_fold_noalloc.restype = ctypes.c_int
+    L.vx_hash_fold_noalloc.argtypes = [_vp, _u64, _u64, _vp, _vp]
     L.vx_probe_alu.restype = ctypes.c_int
     L.vx_probe_alu.argtypes = [ctypes.c_int, _u32, _u32, _vp, _sz, _vp, ctypes.POINTER(_u64)]
     L.vx_plot_info.restype = ctypes.c_int
@@ -386,6 +388,12 @@ class Plot:
         with self._dev():
             self._check(self._L.vx_hash_range(self._h, nonce_begin, count, out.data_ptr(), self._sp(stream)))
         return out
+
+    def hash_fold_noalloc(self, nonce_begin: int, count: int, out, stream=None):
+        """vx_hash_fold_noalloc: xor of H(n) over the range -> out[0] (a 1-element int64 CUDA tensor the caller
+        owns); the library's scratch is a static device array, nothing is allocated."""
+        with self._dev():
+            self._check(self._L.vx_hash_fold_noalloc(self._h, nonce_begin, count, out.data_ptr(), self._sp(stream)))
 
     def hash_sink(self, count: int, sink, stream=None):
         with self._dev():

@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvx.so")
-SOURCES = ["vx_api.cu", "vx_stage1.cu", "vx_stage2.cu", "vx_egress.cu", "vx_probe.cu"]
+SOURCES = ["vx_api.cu", "vx_stage1.cu", "vx_stage2.cu", "vx_egress.cu", "vx_probe.cu", "vx_noalloc.cu"]
 HEADERS = ["vx_internal.h", "vx_blake3.cuh", os.path.join("..", "..", "include", "vx.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "--cudart", "shared"]

@@ -187,6 +187,10 @@ static vx_status sync_and_check(vx_plot *p)
     return VX_OK;
 }
 
+const VxHashConst &vx_plot_hash_const(const vx_plot *p) { return p->hc; }
+int vx_plot_fail(vx_plot *p, int status, const char *what) { return fail(p, (vx_status)status, what); }
+int vx_plot_fail_cuda(vx_plot *p, cudaError_t e, const char *what) { return fail_cuda(p, e, what); }
+
 // ------------------------------------------------------------------------------ the ABI
 extern "C" {
 

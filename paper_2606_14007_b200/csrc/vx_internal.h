@@ -94,6 +94,12 @@ struct VxCtrl {
 #define VX_CHECK(ctrl, cond) do { } while (0)
 #endif
 
+// accessors of the opaque handle (vx_api.cu) for the other .cu files: its folded hash constants, and its
+// error text set the way every ABI call sets it
+struct vx_plot;
+const VxHashConst &vx_plot_hash_const(const vx_plot *p);
+int vx_plot_fail(vx_plot *p, int status, const char *what);                 // returns status (a vx_status)
+int vx_plot_fail_cuda(vx_plot *p, cudaError_t e, const char *what);         // returns VX_ERR_CUDA
 // returns false if (K, B) is not a supported geometry
 bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force_big_tiles, uint32_t passes_log = 0);
 void vx_geom_select_pass(VxGeom *g, uint32_t pass);
