@@ -59,6 +59,28 @@ struct VxS2Params {
 #define VX_ST_VAL ((1ull << 62) - 1)
 #define VX_FULL 0xffffffffu
 
+#ifndef VX_EXP_TMA
+#define VX_EXP_TMA 0
+#endif
+#if VX_EXP_TMA
+// experiment (DESIGN.md 6.2 "TMA staging"): the partition comes into shared memory by cp.async.bulk with an
+// mbarrier, in two halves through the (then free) sorted-key array, instead of by per-thread global loads
+__device__ __forceinline__ uint32_t vx_smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void vx_mbar_init(void *bar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(vx_smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void vx_tma_load(void *dst, const void *src, uint32_t bytes, void *bar) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(vx_smem_addr(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(vx_smem_addr(dst)), "l"(src), "r"(bytes), "r"(vx_smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void vx_mbar_wait(void *bar, uint32_t parity) {
+    asm volatile("{\n.reg .pred p;\nVX_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra VX_DONE;\nbra VX_WAIT;\nVX_DONE:\n}"
+                 :: "r"(vx_smem_addr(bar)), "r"(parity) : "memory");
+}
+#endif
+
 __device__ __forceinline__ uint32_t vx_warp_incl_scan(uint32_t v, int lane)
 {
 #pragma unroll
@@ -177,6 +199,12 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     uint32_t *sub = E;                                  // phases C-D only: 32-bit ranking sub-keys
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_tile, s_tie, s_cnt;
+#if VX_EXP_TMA
+    __shared__ __align__(8) unsigned long long s_mbar;
+    uint32_t par = 0;                                   // phase parity of s_mbar, the same in every thread
+    constexpr uint32_t VX_HALF = CAPA / 2;              // records per staging chunk: the sorted-key array holds half a tile
+    if (threadIdx.x == 0) vx_mbar_init(&s_mbar);        // (the barrier at the top of the tile loop publishes it)
+#endif
     __shared__ unsigned long long s_base2;
     // deferred emit (phase H of tile t runs after phase A of the CTA's next tile): Table-2 prefix at
     // the first record of every bucket of tile t, saved before the bins are recycled
@@ -295,6 +323,12 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
         uint32_t M = 0;
         bool finished = false;
         for (;;) {
+#if VX_EXP_TMA
+            if constexpr (!WIDE) {
+                if (tid == 0 && s_cnt)                  // first half of the partition -> the sorted-key array (free here)
+                    vx_tma_load(keyS, q.part + (size_t)s_tile * q.cap, min(s_cnt, VX_HALF) * 16u, &s_mbar);
+            }
+#endif
             for (int i = tid; i < (int)(VX_NBINS + 32) / 4; i += THREADS)
                 reinterpret_cast<uint4 *>(bins)[i] = make_uint4(0u, 0u, 0u, 0u);
             __syncthreads();
@@ -310,6 +344,38 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
             }
 
             // ---- A. load + bin count -----------------------------------------------------------
+#if VX_EXP_TMA
+            if constexpr (!WIDE) {
+                const uint4 *stage = reinterpret_cast<const uint4 *>(keyS);
+                if (cnt) { vx_mbar_wait(&s_mbar, par); par ^= 1u; }
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    const uint32_t idx = it * THREADS + tid;
+                    key[it] = 0ull; non[it] = 0u;
+                    if (idx < cnt && idx < VX_HALF) {
+                        const uint4 r = stage[idx];
+                        key[it] = ((uint64_t)r.y << 32) | r.x;
+                        non[it] = r.z;
+                    }
+                }
+                if (cnt > VX_HALF) {                    // CTA-uniform
+                    __syncthreads();                    // everybody has taken its records of the first half
+                    if (tid == 0) vx_tma_load(keyS, src + VX_HALF, (cnt - VX_HALF) * 16u, &s_mbar);
+                    vx_mbar_wait(&s_mbar, par); par ^= 1u;
+#pragma unroll
+                    for (int it = 0; it < ITEMS; it++) {
+                        const uint32_t idx = it * THREADS + tid;
+                        if (idx < cnt && idx >= VX_HALF) {
+                            const uint4 r = stage[idx - VX_HALF];
+                            key[it] = ((uint64_t)r.y << 32) | r.x;
+                            non[it] = r.z;
+                        }
+                    }
+                }
+                __syncthreads();                        // staging read; phase C may write the sorted keys
+            } else
+#endif
+            {
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
                 const uint32_t idx = it * THREADS + tid;
@@ -321,6 +387,7 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     key[it] = ((uint64_t)r.y << 32) | r.x;
                     non[it] = r.z;
                 }
+            }
             }
 #pragma unroll
             for (int it = 0; it < ITEMS; it++) {
