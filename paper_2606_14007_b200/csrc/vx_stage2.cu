@@ -263,7 +263,20 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key
                             const uint64_t ni = ((keyS[i] & q.lowmask) << q.nlo_bits) | nonS[i];
                             const unsigned long long at = base2 + e0;
-                            for (uint32_t t = 0; t < cmax; t++)
+                            // the first two successors unconditionally (positions up to CAPA + 1 lie inside the
+                            // arrays' padding), their loads issued together; longer runs take the loop
+                            uint64_t kj[2];
+                            uint32_t bj[2];
+#pragma unroll
+                            for (uint32_t t = 0; t < 2; t++) { kj[t] = keyS[i + 1 + t]; bj[t] = nonS[min(i + 1 + t, (uint32_t)CAPA - 1u)]; }
+#pragma unroll
+                            for (uint32_t t = 0; t < 2; t++)
+                                if (t < c) {
+                                    const uint64_t nj = ((kj[t] & q.lowmask) << q.nlo_bits) | bj[t];
+                                    q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
+                                    q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
+                                }
+                            for (uint32_t t = 2; t < cmax; t++)
                                 if (t < c) {
                                     const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << q.nlo_bits) | nonS[i + 1 + t];
                                     q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
