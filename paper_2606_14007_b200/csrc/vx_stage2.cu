@@ -265,18 +265,18 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             const unsigned long long at = base2 + e0;
                             // the first two successors unconditionally (positions up to CAPA + 1 lie inside the
                             // arrays' padding), their loads issued together; longer runs take the loop
-                            uint64_t kj[2];
-                            uint32_t bj[2];
+                            uint64_t kj[4];
+                            uint32_t bj[4];
 #pragma unroll
-                            for (uint32_t t = 0; t < 2; t++) { kj[t] = keyS[i + 1 + t]; bj[t] = nonS[min(i + 1 + t, (uint32_t)CAPA - 1u)]; }
+                            for (uint32_t t = 0; t < 4; t++) { kj[t] = keyS[i + 1 + t]; bj[t] = nonS[min(i + 1 + t, (uint32_t)CAPA - 1u)]; }
 #pragma unroll
-                            for (uint32_t t = 0; t < 2; t++)
+                            for (uint32_t t = 0; t < 4; t++)
                                 if (t < c) {
                                     const uint64_t nj = ((kj[t] & q.lowmask) << q.nlo_bits) | bj[t];
                                     q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
                                     q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
                                 }
-                            for (uint32_t t = 2; t < cmax; t++)
+                            for (uint32_t t = 4; t < cmax; t++)
                                 if (t < c) {
                                     const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << q.nlo_bits) | nonS[i + 1 + t];
                                     q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
