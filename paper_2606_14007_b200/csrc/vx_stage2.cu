@@ -260,27 +260,32 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
                     if (cmax) {
                         if constexpr (WIDE) {
-                            // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key
-                            const uint64_t ni = ((keyS[i] & q.lowmask) << q.nlo_bits) | nonS[i];
-                            const unsigned long long at = base2 + e0;
-                            // the first two successors unconditionally (positions up to CAPA + 1 lie inside the
+                            // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key.  pb <= 24,
+                            // so only the LOW key word is needed and everything is 32-bit arithmetic:
+                            // h = key_lo & lowmask; nonce_lo = h << tile_log | b; nonce_hi = h >> (32 - tile_log)
+                            const uint32_t *k32 = reinterpret_cast<const uint32_t *>(keyS);
+                            const uint32_t lm = (uint32_t)q.lowmask, nlo = q.nlo_bits;
+                            const uint32_t hi_ = k32[2 * i] & lm;
+                            const uint32_t ni = (hi_ << nlo) | nonS[i], nih = hi_ >> (32u - nlo);
+                            uint2 *dst = q.t2_rec + (base2 + e0);
+                            uint8_t *dsth = q.t2_hi + (base2 + e0);
+                            // the first four successors unconditionally (positions up to CAPA + 3 lie inside the
                             // arrays' padding), their loads issued together; longer runs take the loop
-                            uint64_t kj[4];
-                            uint32_t bj[4];
+                            uint32_t kj[4], bj[4];
 #pragma unroll
-                            for (uint32_t t = 0; t < 4; t++) { kj[t] = keyS[i + 1 + t]; bj[t] = nonS[min(i + 1 + t, (uint32_t)CAPA - 1u)]; }
+                            for (uint32_t t = 0; t < 4; t++) { kj[t] = k32[2 * (i + 1 + t)]; bj[t] = nonS[min(i + 1 + t, (uint32_t)CAPA - 1u)]; }
 #pragma unroll
                             for (uint32_t t = 0; t < 4; t++)
                                 if (t < c) {
-                                    const uint64_t nj = ((kj[t] & q.lowmask) << q.nlo_bits) | bj[t];
-                                    q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
-                                    q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
+                                    const uint32_t h = kj[t] & lm;
+                                    dst[t] = make_uint2(ni, (h << nlo) | bj[t]);
+                                    dsth[t] = (uint8_t)(nih | ((h >> (32u - nlo)) << 4));
                                 }
                             for (uint32_t t = 4; t < cmax; t++)
                                 if (t < c) {
-                                    const uint64_t nj = ((keyS[i + 1 + t] & q.lowmask) << q.nlo_bits) | nonS[i + 1 + t];
-                                    q.t2_rec[at + t] = make_uint2((uint32_t)ni, (uint32_t)nj);
-                                    q.t2_hi[at + t] = (uint8_t)((ni >> 32) | ((nj >> 32) << 4));
+                                    const uint32_t h = k32[2 * (i + 1 + t)] & lm;
+                                    dst[t] = make_uint2(ni, (h << nlo) | nonS[i + 1 + t]);
+                                    dsth[t] = (uint8_t)(nih | ((h >> (32u - nlo)) << 4));
                                 }
                         } else {
                             const uint32_t ni = nonS[i];
