@@ -269,6 +269,12 @@ vx_status vx_device_tables(vx_plot *p, const void **dev_t1_records, const uint64
  * and so send the tile through its "redo with exact (H, n) ranks" path (taken by about 8 tiles of
  * a K = 31 plot otherwise) -- results are identical by construction; tests use it to run that path. */
 #define VX_OPT_SUBKEY_BITS 4
+/* VX_OPT_STAGE2_KERNEL (0, default: the fused kernel whose phases are separated by CTA-wide barriers; 1: the
+ * warp-local variant, in which from the scatter on every warp finishes its own hash range of the tile alone,
+ * wherever it applies -- narrow layout, a warp's range a whole number of buckets: K = 27 .. 32 at B = 24 -- and
+ * the default kernel elsewhere).  Results are identical; the variant measured slower and is kept
+ * as a measured alternative.  Tests and measurements use the option to run both. */
+#define VX_OPT_STAGE2_KERNEL 5
 vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value);
 
 /* Synchronises; any output pointer may be NULL.  max_bucket = largest Table-1 bucket. */

@@ -18,6 +18,7 @@ VX_OPT_FORCE_EXACT_RANK = 1
 VX_OPT_PARTITION_CAPACITY_LIMIT = 2
 VX_OPT_TABLE2_CAPACITY_LIMIT = 3
 VX_OPT_SUBKEY_BITS = 4
+VX_OPT_STAGE2_KERNEL = 5
 VX_TABLE2_REKEYED = 3
 VX_CREATE_WIDE_LAYOUT = 1
 VX_CREATE_BIG_TILES = 2

@@ -73,6 +73,7 @@ bool vx_geom_init(VxGeom *g, uint32_t K, uint32_t B, bool force_wide, bool force
     g->t2_cap = (g->N >> passes_log) + (1u << 16);        // per pass
     g->t2_check = g->t2_cap;
     g->subkey_bits = 32;
+    g->s2_kernel = 0;
     g->rec1_bytes = g->nonce_size + 8;
     g->rec2_bytes = 2 * g->nonce_size;
     size_t o = 0;
@@ -761,6 +762,10 @@ vx_status vx_plot_set_option(vx_plot *p, int option, uint64_t value)
     case VX_OPT_SUBKEY_BITS:
         if (value > 32) return fail(p, VX_ERR_ARG, "sub-key bits outside [0, 32]");
         p->g.subkey_bits = (uint32_t)value;
+        return VX_OK;
+    case VX_OPT_STAGE2_KERNEL:
+        if (value > 1) return fail(p, VX_ERR_ARG, "stage-2 kernel choice outside [0, 1]");
+        p->g.s2_kernel = (uint32_t)value;
         return VX_OK;
     }
     return fail(p, VX_ERR_ARG, "unknown option");

@@ -38,6 +38,7 @@ struct VxGeom {
     uint64_t t2_check;    // = t2_cap; likewise for Table 2
     uint32_t subkey_bits; // = 32: hash bits below the bin index that stage 2's fast ranking compares; a test hook
                           // narrows it so that the tie -> exact re-rank path of a tile runs under test
+    uint32_t s2_kernel;   // 0: the classic fused kernel; 1: the warp-local variant where it applies (VX_OPT_STAGE2_KERNEL)
     uint64_t N;    // 2^K
     uint64_t P;    // partitions resident at a time: 2^(pb - passes_log)
     uint64_t NB;   // 2^B

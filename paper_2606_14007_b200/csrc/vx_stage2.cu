@@ -683,6 +683,423 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     if (lane == 0 && cta_max_bucket) atomicMax(&q.ctrl->max_bucket, cta_max_bucket);
 }
 
+// ------------------------------------------------------------------------------ warp-local variant
+// vx_k_sort_match_wl: the same tile, the same phases A-C and the same arrays as vx_k_sort_match, but from the
+// scatter on every WARP finishes its own share of the tile alone.  After phase C the records are grouped by bin
+// and bins ascend with the hash, so warp w owns the bins [w * BPW, (w + 1) * BPW), BPW = bins / warps, i.e.
+// the contiguous sorted positions [S, Send) = [bins[w * BPW], bins[(w + 1) * BPW]) -- a whole number of buckets
+// when fb >= log2(warps), so no match crosses into another warp's range (matching is per bucket).
+// The warp ranks its bins (D), counts its matches (E), scans them (F) and writes its records and bucket offsets
+// back (G) behind __syncwarp only: the five CTA-wide barriers D|rewrite|E|F|F'|G of the classic kernel go, the
+// warps of a CTA drift apart and fill each other's shared-memory latencies.  The tile total for the look-back
+// is published by the last warp to finish its scan.  The Table-2 prefix E[] is relative to the warp's range;
+// the warp's offset inside the tile is the sum of the totals of the warps before it, added in the emit (H),
+// which the owning warp runs over its own range as well (deferred behind the next tile's phase A, as before).
+// Applies to the narrow layout with matching on, log2(warps) <= fb <= 9 (K = 27 .. 32 at B = 24).  Same results
+// bit for bit (tests/test_gpu_stage2_kernels.py runs every eligible geometry through both kernels).
+// MEASURED AND NOT THE DEFAULT (DESIGN.md 6.2 "warp-local phases", profiles/r02_warp_local.md): K=31 33.9 ms
+// against 30.0, K=32 71.2 against 64.7 -- 30 % more warp instructions (the bin-aligned runs of phase D, the
+// dynamic loops) and the same share of barrier stalls, now all on the three barriers left (the warps' ranges
+// differ by +-6 %, and the look-back wait grew).  Runs only with VX_OPT_STAGE2_KERNEL = 1.
+template <int THREADS, int ITEMS, int BIN_BITS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+vx_k_sort_match_wl(const __grid_constant__ VxS2Params q)
+{
+    constexpr uint32_t VX_NBINS = 1u << BIN_BITS;
+    constexpr int CAPA = THREADS * ITEMS;
+    constexpr int WARPS = THREADS / 32;
+    constexpr uint32_t BPW = VX_NBINS / WARPS;          // bins per warp
+    constexpr uint32_t VX_SCAN_L = 11;                  // positions per lane and round of the warp's scan (odd)
+    extern __shared__ __align__(16) uint8_t vx_smem[];
+    uint64_t *keyS = (uint64_t *)vx_smem;               // the layout of vx_k_sort_match
+    uint32_t *nonS = (uint32_t *)(keyS + CAPA + 8);
+    uint32_t *bins = nonS + CAPA;
+    uint32_t *E = bins + VX_NBINS + 32;                 // match-count prefix, relative to the owning warp's range
+    uint32_t *sub = E;                                  // phases C-D: ranking keys
+    __shared__ uint32_t s_warp[32];
+    __shared__ uint32_t s_tile, s_tie, s_cnt;
+    __shared__ uint32_t s_done, s_M;                    // warps that have finished F; sum of their totals
+    __shared__ uint32_t s_Mw[WARPS];                    // per-warp totals (read again by the deferred emit)
+    __shared__ unsigned long long s_base2;
+    constexpr uint32_t VX_DEFER_MAXB = 512;
+    __shared__ uint32_t s_e2[VX_DEFER_MAXB];            // Table-2 prefix (warp-relative) at the first record of every bucket
+    __shared__ uint32_t s_p[3];                         // tile, count, matches of the tile whose emit is pending
+
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int sh = q.binshift - 32;
+    const uint32_t submask = q.submask;
+    const uint64_t Tm1 = q.Tm1;
+    const uint64_t bmask = q.bmask;
+    uint32_t cta_max_bucket = 0;
+    const uint32_t nb_local = 1u << q.fb;
+    const uint32_t nbw = nb_local / WARPS;              // buckets per warp (>= 1: checked at launch)
+    const int bsh = BIN_BITS - (int)q.fb;               // first bin of local bucket bl = bl << bsh
+    bool pending = false;
+    uint32_t pS = 0, pEnd = 0;                          // the warp's range in the pending tile (warp-uniform)
+
+    // ---- look-back for the Table-2 base, then H over the warp's own range
+    auto lookback_emit = [&](uint32_t tile, uint32_t M) {
+        if (tid < 32) {
+            const unsigned long long b2 = vx_lookback(q.status, tile, M, lane);
+            if (tid == 0) {
+                s_base2 = b2;
+                if (tile == q.tile_end - 1 && q.slice_end_out) *q.slice_end_out = b2 + M;
+            }
+        }
+        __syncthreads();
+        const unsigned long long base2 = s_base2;
+        // totals of the warps before this one
+        const uint32_t mw = lane < w ? s_Mw[lane] : 0u;
+        const uint32_t Ow = __reduce_add_sync(VX_FULL, mw);
+        if (base2 + M > q.t2_cap) {
+            if (tid == 0) atomicOr(&q.ctrl->flags, VX_FLAG_T2_OVERFLOW);
+        } else {
+            const uint32_t Mw = s_Mw[w];
+            uint2 *t2 = q.t2_rec + (base2 + Ow);
+            for (uint32_t p0 = pS; p0 < pEnd; p0 += 32) {
+                const uint32_t i = p0 + lane;
+                uint32_t e0 = 0, c = 0;
+                if (i < pEnd) {
+                    e0 = E[i];
+                    c = (i + 1 < pEnd ? E[i + 1] : Mw) - e0;
+                    VX_CHECK(q.ctrl, e0 + c <= Mw && (c == 0 || i + c < pEnd) && base2 + Ow + e0 + c <= q.t2_cap);
+                }
+                const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
+                if (cmax) {
+                    const uint32_t ni = nonS[min(i, (uint32_t)CAPA - 1u)];
+                    const uint32_t *np = nonS + i + 1;
+                    uint2 *dst = t2 + e0;
+#pragma unroll
+                    for (uint32_t t = 0; t < 4; t++)
+                        if (t < c) dst[t] = make_uint2(ni, np[t]);
+                    for (uint32_t t = 4; t < cmax; t++)
+                        if (t < c) dst[t] = make_uint2(ni, np[t]);
+                }
+            }
+        }
+        const unsigned long long pg0 = (unsigned long long)tile << q.fb;
+        for (uint32_t j = lane; j < nbw; j += 32) {
+            const uint32_t bl = (uint32_t)w * nbw + j;
+            q.t2_off[pg0 + bl] = base2 + Ow + s_e2[bl];
+        }
+        if (tile == q.P - 1 && tid == 0) {
+            q.t2_off[q.NB] = base2 + M;
+            q.ctrl->t2_total = base2 + M;
+        }
+    };
+
+    for (;;) {
+        // (no barrier here: a tile ends with one, and s_tile / s_cnt are read behind the next)
+        if (tid == 0) {
+            const uint32_t t = q.tile_begin + atomicAdd(&q.ctrl->ticket, 1u);
+            s_tile = t;
+            s_cnt = t < q.tile_end ? min(q.cursor[t], q.cap_check) : 0u;
+            const uint32_t pf = t + gridDim.x;          // bulk L2 prefetch of a partition taken a round later
+            if (pf < q.tile_end) {
+                const uint32_t n = min(q.cursor[pf], q.cap_check);
+                const char *p = reinterpret_cast<const char *>(q.part) + (size_t)pf * q.cap * 16;
+                const uint32_t bytes = n * 16u;
+                if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(p), "r"(bytes) : "memory");
+            }
+        }
+        uint32_t exact = q.force_exact;
+        uint32_t tile, cnt;
+        uint32_t S = 0, Send = 0;
+        bool finished = false;
+        for (;;) {
+            uint4 *src;
+            uint64_t key[ITEMS];
+            uint32_t non[ITEMS], sn[ITEMS];
+            for (int i = tid; i < (int)(VX_NBINS + 32) / 4; i += THREADS)
+                reinterpret_cast<uint4 *>(bins)[i] = make_uint4(0u, 0u, 0u, 0u);
+            __syncthreads();
+            if (tid == 0) { s_tie = 0u; s_done = 0u; s_M = 0u; }
+            tile = s_tile;
+            const bool valid = tile < q.tile_end;
+            cnt = s_cnt;
+            src = q.part + (size_t)tile * q.cap;
+            // ---- A. load + bin count -----------------------------------------------------------
+#pragma unroll
+            for (int it = 0; it < ITEMS; it++) {
+                const uint32_t idx = it * THREADS + tid;
+                const uint4 r = idx < cnt ? __ldcs(src + idx) : make_uint4(0u, 0u, 0u, 0u);
+                key[it] = ((uint64_t)r.y << 32) | r.x;
+                non[it] = r.z;
+            }
+#pragma unroll
+            for (int it = 0; it < ITEMS; it++) {
+                const uint32_t idx = it * THREADS + tid;
+                VX_CHECK(q.ctrl, cnt <= (uint32_t)CAPA && cnt <= q.cap && vx_bin<VX_NBINS>(key[it], sh) < VX_NBINS);
+                if (idx < cnt) sn[it] = atomicAdd(&bins[vx_bin<VX_NBINS>(key[it], sh)], 1u);
+            }
+            if (pending) {                              // the previous tile of this CTA: look-back + H
+                lookback_emit(s_p[0], s_p[2]);
+                pending = false;
+            }
+            if (!valid) { finished = true; break; }
+            __syncthreads();
+            // ---- B. scan -------------------------------------------------------------------------
+            {
+                const uint32_t total = vx_block_exscan<THREADS, VX_NBINS / THREADS>(bins, s_warp);
+                if (tid == 0) bins[VX_NBINS] = total;
+            }
+            __syncthreads();
+            // ---- C. scatter to bin start + slot --------------------------------------------------
+            {
+                uint32_t pos[ITEMS];
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    const uint32_t idx = it * THREADS + tid;
+                    pos[it] = idx < cnt ? bins[vx_bin<VX_NBINS>(key[it], sh)] + sn[it] : 0xffffffffu;
+                }
+#pragma unroll
+                for (int it = 0; it < ITEMS; it++) {
+                    if (pos[it] != 0xffffffffu) {
+                        VX_CHECK(q.ctrl, pos[it] < cnt);
+                        keyS[pos[it]] = key[it];
+                        nonS[pos[it]] = non[it];
+                        sub[pos[it]] = (vx_subkey(key[it], sh) & submask) | sn[it];
+                        if (sn[it] > 15u) s_tie = 1u;   // a bin of more than 16 records: rank it exactly
+                    }
+                }
+            }
+            if (tid < 8) keyS[cnt + tid] = ~0ull;       // sentinels behind the last record
+            __syncthreads();
+            // a bin of more than 16 records: the slot no longer fits the ranking key's low bits, the fast ranks
+            // could collide; nothing has been written yet -> the tile starts again with exact ranks
+            if (!exact && s_tie) {
+                if (tid == 0) atomicAdd(&q.ctrl->retries, 1u);
+                exact = 1u;
+                continue;
+            }
+            // ======== from here to the barrier at the end the warp works alone on [S, Send) ==========
+            S = bins[(uint32_t)w * BPW];
+            Send = bins[(uint32_t)w * BPW + BPW];
+            VX_CHECK(q.ctrl, S <= Send && Send <= cnt);
+            // ---- D. rank inside multi-record bins, a run of whole bins (<= 32 positions) at a time, in place
+            {
+                uint32_t b0 = (uint32_t)w * BPW, p0 = S;
+                const uint32_t b_hi = b0 + BPW;
+                while (b0 < b_hi) {                     // warp-uniform
+                    // ends of the next 64 bins; the run takes those that end within 32 positions of p0
+                    const uint32_t ia = b0 + 1 + lane, ib = ia + 32;
+                    const uint32_t ea = ia <= b_hi ? bins[ia] : 0xffffffffu;
+                    const uint32_t eb = ib <= b_hi ? bins[ib] : 0xffffffffu;
+                    const uint32_t nb = __popc(__ballot_sync(VX_FULL, ea - p0 <= 32u)) +
+                                        __popc(__ballot_sync(VX_FULL, eb - p0 <= 32u));
+                    if (nb == 0) {
+                        // a single bin of more than 32 records (never with real hashes): one lane sorts it by (H, n)
+                        const uint32_t p1 = __shfl_sync(VX_FULL, ea, 0);
+                        if (lane == 0) {
+                            for (uint32_t a = p0 + 1; a < p1; a++) {
+                                const uint64_t k = keyS[a];
+                                const uint32_t nn = nonS[a];
+                                uint32_t c = a;
+                                while (c > p0 && (keyS[c - 1] > k || (keyS[c - 1] == k && nonS[c - 1] > nn))) {
+                                    keyS[c] = keyS[c - 1]; nonS[c] = nonS[c - 1]; c--;
+                                }
+                                keyS[c] = k; nonS[c] = nn;
+                            }
+                        }
+                        __syncwarp();
+                        b0 += 1; p0 = p1;
+                        continue;
+                    }
+                    const uint32_t p1 = nb <= 32u ? __shfl_sync(VX_FULL, ea, (nb - 1u) & 31u)
+                                                  : __shfl_sync(VX_FULL, eb, (nb - 33u) & 31u);
+                    const uint32_t i = p0 + lane;
+                    const bool act = i < p1;
+                    uint64_t k = 0ull;
+                    uint32_t nn = 0u, s = 0u, n = 0u;
+                    if (act) {
+                        k = keyS[i];
+                        nn = nonS[i];
+                        const uint32_t b = vx_bin<VX_NBINS>(k, sh);
+                        s = bins[b];
+                        n = bins[b + 1] - s;
+                        VX_CHECK(q.ctrl, b >= b0 && b < b0 + nb && s <= i && i < s + n && s + n <= p1);
+                        if (n == 1u) n = 0u;            // alone in its bin: stays
+                    }
+                    const uint32_t nm = __reduce_max_sync(VX_FULL, n);
+                    if (nm) {                           // warp-uniform: some bin of the run holds several records
+                        uint32_t rank = 0;
+                        if (!exact) {
+                            const uint32_t *sp = sub + s;
+                            const uint32_t ks = act ? sub[i] : 0u;
+#pragma unroll
+                            for (uint32_t j = 0; j < 4; j++) {
+                                const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
+                                rank += kj < ks ? 1u : 0u;
+                            }
+                            if (nm > 4) {
+#pragma unroll 1
+                                for (uint32_t j = 4; j < nm; j++) {
+                                    const uint32_t kj = j < n ? sp[j] : 0xffffffffu;
+                                    rank += kj < ks ? 1u : 0u;
+                                }
+                            }
+                        } else {                        // by (H, n), reading A10
+                            const uint64_t *kp = keyS + s;
+                            const uint32_t *np = nonS + s;
+#pragma unroll 1
+                            for (uint32_t j = 0; j < nm; j++)
+                                if (j < n) rank += (kp[j] < k || (kp[j] == k && np[j] < nn)) ? 1u : 0u;
+                        }
+                        __syncwarp();                   // every lane has read its record and its bin
+                        if (n) {
+                            VX_CHECK(q.ctrl, s + rank < p1);
+                            keyS[s + rank] = k;
+                            nonS[s + rank] = nn;
+                        }
+                    }
+                    b0 += nb; p0 = p1;
+                }
+            }
+            __syncwarp();
+            // ---- E. match count: lane i counts its successors within reach ------------------------
+            {
+                const uint32_t last = cnt ? cnt - 1 : 0u;
+                const bool guarded = tile == q.P - 1;   // lim can reach the sentinel value ~0 only in the last tile
+                constexpr int VX_EB = 3;
+                for (uint32_t g0 = S; g0 < Send; g0 += 32u * VX_EB) {
+                    if (!guarded) {
+                        uint64_t ki[VX_EB], lim[VX_EB], kn[VX_EB];
+                        uint32_t pos[VX_EB];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            // lanes behind the range read inside the arrays (results unused)
+                            const uint32_t i = min(g0 + 32u * u + lane, (uint32_t)CAPA);
+                            ki[u] = keyS[i];
+                            kn[u] = keyS[i + 1];
+                            pos[u] = i;
+                        }
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            lim[u] = min(ki[u] + Tm1, ki[u] | bmask);
+                            // the fast pass is valid iff the keys came out strictly increasing (the first key of the
+                            // next warp's range lies in a later bin: larger by construction)
+                            if (!exact && pos[u] + 1 < Send && kn[u] <= ki[u]) s_tie = 1u;
+                        }
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) kn[u] = keyS[pos[u] + 4];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) if (kn[u] <= lim[u]) pos[u] += 4;
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) kn[u] = keyS[pos[u] + 2];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) if (kn[u] <= lim[u]) pos[u] += 2;
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) kn[u] = keyS[pos[u] + 1];
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) if (kn[u] <= lim[u]) pos[u] += 1;
+#pragma unroll
+                        for (int u = 0; u < VX_EB; u++) {
+                            const uint32_t i = g0 + 32u * u + lane;
+                            uint32_t c = i < Send ? pos[u] - i : 0u;
+                            if (__any_sync(VX_FULL, c == 7u)) {
+                                for (uint32_t j = i + 8;; j++) {
+                                    const bool m = c >= 7u && j < cnt && keyS[min(j, last)] <= lim[u];
+                                    c += m ? 1u : 0u;
+                                    if (!__any_sync(VX_FULL, m)) break;
+                                }
+                            }
+                            VX_CHECK(q.ctrl, c == 0 || i + c < Send);
+                            if (i < Send) E[i] = c;
+                        }
+                    } else {
+#pragma unroll 1
+                        for (int u = 0; u < VX_EB; u++) {
+                            const uint32_t i = g0 + 32u * u + lane;
+                            const bool in = i < Send;
+                            const uint64_t ki = keyS[min(i, (uint32_t)CAPA)];
+                            uint64_t lim = ki + Tm1;
+                            if (lim < ki) lim = ~0ull;
+                            lim = min(lim, ki | bmask);
+                            uint32_t c = 0;
+                            if (!exact && i + 1 < Send && keyS[i + 1] <= ki) s_tie = 1u;
+                            for (uint32_t j = i + 1;; j++) {
+                                const bool m = in && j < cnt && keyS[min(j, last)] <= lim;
+                                c += m ? 1u : 0u;
+                                if (!__any_sync(VX_FULL, m)) break;
+                            }
+                            VX_CHECK(q.ctrl, c == 0 || i + c < Send);
+                            if (in) E[i] = c;
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            // ---- F. exclusive scan of the warp's counts, VX_SCAN_L consecutive positions per lane and round
+            //         (an odd stride: conflict-free); the last warp to get here publishes the tile's total
+            uint32_t Mw = 0;
+            for (uint32_t base = S; base < Send; base += 32u * VX_SCAN_L) {
+                const uint32_t n = min(Send - base, 32u * VX_SCAN_L);
+                const uint32_t L = ((n + 31u) >> 5) | 1u;
+                const uint32_t o = (uint32_t)lane * L;
+                uint32_t v[VX_SCAN_L];
+                uint32_t sum = 0;
+#pragma unroll
+                for (uint32_t kk = 0; kk < VX_SCAN_L; kk++) {
+                    const uint32_t t = (kk < L && o + kk < n) ? E[base + o + kk] : 0u;
+                    v[kk] = sum;
+                    sum += t;
+                }
+                const uint32_t incl = vx_warp_incl_scan(sum, lane);
+                const uint32_t off = Mw + incl - sum;
+#pragma unroll
+                for (uint32_t kk = 0; kk < VX_SCAN_L; kk++)
+                    if (kk < L && o + kk < n) E[base + o + kk] = v[kk] + off;
+                Mw += __shfl_sync(VX_FULL, incl, 31);
+            }
+            __syncwarp();
+            if (lane == 0) {
+                s_Mw[w] = Mw;
+                atomicAdd(&s_M, Mw);
+                __threadfence_block();
+                if (atomicAdd(&s_done, 1u) == (uint32_t)WARPS - 1u) {
+                    __threadfence_block();
+                    const uint32_t M = *(volatile uint32_t *)&s_M;
+                    // a tile that will be redone (its fast ranking met a tie) publishes nothing
+                    if ((exact || *(volatile uint32_t *)&s_tie == 0u) && tile)
+                        ((volatile unsigned long long *)q.status)[tile] = VX_ST_AGG | M;
+                }
+            }
+            // ---- G. the warp's records back in place; CSR offsets of Table 1 for its buckets -----------
+            for (uint32_t p = S + lane; p < Send; p += 32) {
+                const uint64_t k = keyS[p];
+                src[p] = make_uint4((uint32_t)k, (uint32_t)(k >> 32), nonS[p], 0u);
+            }
+            {
+                const unsigned long long gb0 = (unsigned long long)tile << q.fb;
+                const unsigned long long base1 = q.part_base[tile];
+                for (uint32_t j = lane; j < nbw; j += 32) {
+                    const uint32_t bl = (uint32_t)w * nbw + j;
+                    const uint32_t s = bins[bl << bsh], e = bins[(bl + 1u) << bsh];
+                    VX_CHECK(q.ctrl, S <= s && s <= e && e <= Send && gb0 + bl < q.NB && bl < VX_DEFER_MAXB);
+                    cta_max_bucket = max(cta_max_bucket, e - s);
+                    q.t1_off[gb0 + bl] = base1 + s;
+                    s_e2[bl] = s < Send ? E[s] : Mw;
+                }
+                if (tile == q.P - 1 && tid == 0) q.t1_off[q.NB] = base1 + cnt;
+            }
+            __syncthreads();
+            if (!exact && s_tie) {                      // block-uniform: redo this tile exactly
+                if (tid == 0) atomicAdd(&q.ctrl->retries, 1u);
+                exact = 1u;
+                continue;
+            }
+            break;
+        }
+        if (finished) break;
+        pending = true;
+        pS = S; pEnd = Send;
+        if (tid == 0) { s_p[0] = tile; s_p[1] = cnt; s_p[2] = s_M; }   // read behind the next tile's barriers
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) cta_max_bucket = max(cta_max_bucket, __shfl_xor_sync(VX_FULL, cta_max_bucket, d));
+    if (lane == 0 && cta_max_bucket) atomicMax(&q.ctrl->max_bucket, cta_max_bucket);
+}
+
 // ------------------------------------------------------------------------------ export
 // Table-1 records [first, first + count) of the CSR numbering, gathered from the partition array
 // into the external format nonce[NS] LE || hash[8] (digest bytes, = H big-endian) in `out`.
@@ -861,6 +1278,16 @@ size_t vx_stage2_smem_bytes(const VxGeom &g)
 
 #define VX_S2_KERNEL(WIDE) vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, VX_TILE_LOG, VX_S2_MINB, WIDE>
 #define VX_S2B_KERNEL(WIDE) vx_k_sort_match<VX_S2B_THREADS, VX_S2B_ITEMS, VX_TILE_LOG_BIG, 1, WIDE>
+#define VX_S2_KERNEL_WL vx_k_sort_match_wl<VX_S2_THREADS, VX_S2_ITEMS, VX_TILE_LOG, VX_S2_MINB>
+#define VX_S2B_KERNEL_WL vx_k_sort_match_wl<VX_S2B_THREADS, VX_S2B_ITEMS, VX_TILE_LOG_BIG, 1>
+
+// the warp-local kernel applies when every warp's share of the bins is a whole number of buckets (no match
+// crosses a warp's range), the bucket starts are bin starts and the deferred emit's bucket table fits
+bool vx_stage2_warp_local(const VxGeom &g, bool do_match)
+{
+    const uint32_t warps_log = g.tile_log == VX_TILE_LOG_BIG ? 5u : 4u;   // 1024 / 512 threads
+    return do_match && !g.wide && g.s2_kernel == 1u && g.fb >= warps_log && g.fb <= 9u;
+}
 
 cudaError_t vx_stage2_configure(void)
 {
@@ -873,6 +1300,8 @@ cudaError_t vx_stage2_configure(void)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, small);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(false), cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2_KERNEL_WL, cudaFuncAttributeMaxDynamicSharedMemorySize, small);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL_WL, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     return e;
 }
 
@@ -932,7 +1361,11 @@ cudaError_t vx_launch_stage2(const VxGeom &g, uint8_t *ws, bool do_match, bool f
     grid = (uint64_t)num_sms * VX_EXP_GRID_PER_SM;
 #endif
     if (grid > tile_end - tile_begin) grid = tile_end - tile_begin;
-    if (big && g.wide) VX_S2B_KERNEL(true)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
+    if (vx_stage2_warp_local(g, do_match)) {
+        if (big) VX_S2B_KERNEL_WL<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
+        else VX_S2_KERNEL_WL<<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
+    }
+    else if (big && g.wide) VX_S2B_KERNEL(true)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
     else if (big) VX_S2B_KERNEL(false)<<<(unsigned)grid, VX_S2B_THREADS, smem, st>>>(q);
     else if (g.wide) VX_S2_KERNEL(true)<<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);
     else VX_S2_KERNEL(false)<<<(unsigned)grid, VX_S2_THREADS, smem, st>>>(q);

@@ -59,8 +59,10 @@ def test_hash_worked_values(vx):
 
 
 # ------------------------------------------------------------------ full tables, small K
-def run_plot(vx, K, key, B, force_exact=False, flags=0, subkey_bits=None, counters=None):
+def run_plot(vx, K, key, B, force_exact=False, flags=0, subkey_bits=None, counters=None, s2_kernel=None):
     plot = vx.Plot(K, key, B, flags=flags)
+    if s2_kernel is not None:
+        plot.set_option(vx.VX_OPT_STAGE2_KERNEL, s2_kernel)
     if force_exact:
         plot.set_option(vx.VX_OPT_FORCE_EXACT_RANK, 1)
     if subkey_bits is not None:
