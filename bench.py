@@ -304,7 +304,13 @@ def run_cuda(args):
     K = args.K
     # independent plots: rank r plots under key SplitMix64(seed_for_K + 1000 r)
     key = vx_inputs.key_from_seed(rank_seed(K, rank))
-    plot = vx.Plot(K, key, BUCKET_BITS, device=dev, flags=args.flags)
+    def new_plot(**kw):
+        p = vx.Plot(K, key, BUCKET_BITS, device=dev, flags=args.flags, **kw)
+        if args.s2_kernel:      # measurement: the warp-local stage-2 kernel instead of the default
+            p.set_option(vx.VX_OPT_STAGE2_KERNEL, args.s2_kernel)
+        return p
+
+    plot = new_plot()
     N = 1 << K
     stream = torch.cuda.current_stream()
 
@@ -372,7 +378,7 @@ def run_cuda(args):
 
         def e2e_step():
             nonlocal d2h
-            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace, flags=args.flags)
+            p2 = new_plot(workspace=plot.workspace)
             moved = 0
             for s in range(passes):
                 p2.select_pass(s)
@@ -404,7 +410,7 @@ def run_cuda(args):
 
         def e2e_step():
             nonlocal d2h
-            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace, flags=args.flags)  # key -> kernel params
+            p2 = new_plot(workspace=plot.workspace)  # key -> kernel params
             p2.build_table1(stream)
             d2h = p2.sort_match_table2_to_host(copy_stream, pinned_rec.data_ptr(), rec_cap, pinned_off.data_ptr(),
                                                slices=args.e2e_slices, stream=stream) + (nb + 1) * 8
@@ -421,7 +427,7 @@ def run_cuda(args):
 
         def e2e_step():
             nonlocal d2h
-            p2 = vx.Plot(K, key, BUCKET_BITS, device=dev, workspace=plot.workspace, flags=args.flags)  # key -> kernel params
+            p2 = new_plot(workspace=plot.workspace)  # key -> kernel params
             p2.build_table1(stream)
             p2.sort_match_table2(stream)
             moved = 0
@@ -502,7 +508,7 @@ def run_cuda(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32/u64",
             "data": "synthetic",
-            "config": make_config(K),
+            "config": dict(make_config(K), **({"stage2_kernel": "warp-local variant (VX_OPT_STAGE2_KERNEL = 1)"} if args.s2_kernel else {})),
             "plot_seconds": ms_per_step * 1e-3, "workspace_GB": plot.workspace_bytes / 1e9,
             "stages": {"build_table1": {"ms": s1, "nonces_per_s": N / (s1 * 1e-3), "roofline": r1},
                        "sort_match_table2": {"ms": s2, "nonces_per_s": N / (s2 * 1e-3), "roofline": r2}},
@@ -693,6 +699,8 @@ def main():
                     help="cpu_baseline: the oracle makes this plot in full (hashing on nproc threads), and K=20 on one")
     ap.add_argument("--flags", type=int, default=0,
                     help="test-only layout flags (1 wide layout, 2 big tiles): ncu captures of the K>=32 geometries at small K")
+    ap.add_argument("--s2-kernel", dest="s2_kernel", type=int, default=0, choices=[0, 1],
+                    help="VX_OPT_STAGE2_KERNEL: 0 = the default fused kernel, 1 = its warp-local variant (a measured alternative)")
     ap.add_argument("--one-plot", dest="one_plot", action="store_true",
                     help="with --gpus N > 1: ONE plot sharded over the N ranks (strong scaling) instead of one plot per rank")
     ap.add_argument("--probe-alu", dest="probe_alu", action="store_true",
