@@ -90,3 +90,56 @@ def test_unknown_kernel_choice_is_rejected(vx):
     with pytest.raises(Exception):
         plot.set_option(vx.VX_OPT_STAGE2_KERNEL, 2)
     plot.free()
+
+
+@pytest.mark.parametrize("K,B,seed,flags,slices", [(14, 9, 5, 0, 3), (16, 12, 1, 0, 16), (20, 16, 3, 0, 7),
+                                                   (22, 16, 7, 0, 64), (18, 12, 9, 2, 5), (22, 16, 7, 2, 16)])
+def test_warp_local_kernel_in_slices_streamed_to_host(vx, K, B, seed, flags, slices):
+    """The warp-local kernel launched as partition-range slices (vx_sort_match_table2_to_host: the look-back
+    state carries over from slice to slice, the last tile of a slice reports the running |Table 2|)."""
+    import torch
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_cached(K, B, seed)
+    plot = vx.Plot(K, key, B, flags=flags)
+    plot.set_option(vx.VX_OPT_STAGE2_KERNEL, 1)
+    copy = torch.cuda.Stream()
+    rec = torch.empty(8 * len(o_n1) + 64, dtype=torch.uint8, pin_memory=True)
+    off = torch.empty((1 << B) + 1, dtype=torch.int64, pin_memory=True)
+    rec.fill_(0xEE); off.fill_(-1)
+    plot.build_table1()
+    got = plot.sort_match_table2_to_host(copy, rec.data_ptr(), rec.numel(), off.data_ptr(), slices=slices)
+    assert got == 8 * len(o_n1)
+    off2 = off.numpy().view(np.uint64)
+    assert np.array_equal(off2, o_t2o)
+    g1, g2 = canon_t2(off2, *decode_t2(rec.numpy()[:got], 4))
+    assert np.array_equal(g1, o_n1) and np.array_equal(g2, o_n2)
+    assert np.all(rec.numpy()[got:] == 0xEE)
+    off1, raw1 = plot.read_tables(1)
+    assert np.array_equal(off1, o_off)
+    assert np.array_equal(raw1, oracle.serialize_t1(4, o_non, o_has))
+    plot.free()
+
+
+@pytest.mark.parametrize("K,B,seed,passes_log", [(16, 12, 1, 1), (20, 16, 3, 2), (22, 18, 8, 1)])
+def test_warp_local_kernel_in_bucket_range_passes(vx, K, B, seed, passes_log):
+    """... and on the passes of a plot made in 2^l bucket-range passes (tile and bucket indices relative to the pass)."""
+    key = vx_inputs.key_from_seed(seed)
+    o_off, o_non, o_has, o_t2o, o_n1, o_n2 = oracle_cached(K, B, seed)
+    plot = vx.Plot(K, key, B, flags=vx.VX_CREATE_PASSES_LOG(passes_log))
+    plot.set_option(vx.VX_OPT_STAGE2_KERNEL, 1)
+    nb = (1 << B) >> passes_log
+    for s in range(1 << passes_log):
+        plot.select_pass(s)
+        plot.build_table1()
+        plot.sort_match_table2()
+        off1, raw1 = plot.read_tables(1)
+        off2, raw2 = plot.read_tables(2)
+        lo, hi = s * nb, (s + 1) * nb
+        assert np.array_equal(off1, o_off[lo:hi + 1] - o_off[lo])
+        a, b = int(o_off[lo]), int(o_off[hi])
+        assert np.array_equal(raw1, oracle.serialize_t1(4, o_non[a:b], o_has[a:b]))
+        assert np.array_equal(off2, o_t2o[lo:hi + 1] - o_t2o[lo])
+        g1, g2 = canon_t2(off2, *decode_t2(raw2, 4))
+        a2, b2 = int(o_t2o[lo]), int(o_t2o[hi])
+        assert np.array_equal(g1, o_n1[a2:b2]) and np.array_equal(g2, o_n2[a2:b2])
+    plot.free()
