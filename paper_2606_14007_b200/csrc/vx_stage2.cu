@@ -197,6 +197,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
     uint32_t *bins = nonS + CAPA;                       // VX_NBINS + 1 (+ pad)
     uint32_t *E = bins + VX_NBINS + 32;                 // CAPA + 1 (+ pad): match-count prefix
     uint32_t *sub = E;                                  // phases C-D only: 32-bit ranking sub-keys
+    // wide layout: bits 32.. of every sorted record's nonce, one byte each (+ pad), filled by phase G for the
+    // emit (which then finds the low 32 nonce bits in nonS, like the narrow one)
+    uint8_t *hiS = (uint8_t *)(E + CAPA + 32);
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_tile, s_tie, s_cnt;
 #if VX_EXP_TMA
@@ -260,32 +263,28 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                     const uint32_t cmax = __reduce_max_sync(VX_FULL, c);
                     if (cmax) {
                         if constexpr (WIDE) {
-                            // nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key.  pb <= 24,
-                            // so only the LOW key word is needed and everything is 32-bit arithmetic:
-                            // h = key_lo & lowmask; nonce_lo = h << tile_log | b; nonce_hi = h >> (32 - tile_log)
-                            const uint32_t *k32 = reinterpret_cast<const uint32_t *>(keyS);
-                            const uint32_t lm = (uint32_t)q.lowmask, nlo = q.nlo_bits;
-                            const uint32_t hi_ = k32[2 * i] & lm;
-                            const uint32_t ni = (hi_ << nlo) | nonS[i], nih = hi_ >> (32u - nlo);
+                            // phase G left the low 32 bits of every sorted record's nonce in nonS and the bits above
+                            // them in hiS: the emit is the narrow one plus a byte of high bits per Table-2 record.
+                            // The first four successors unconditionally (positions up to CAPA + 3 lie inside the
+                            // arrays' padding), their loads issued together ahead of the stores; longer runs take the loop
+                            const uint32_t ni = nonS[i], nih = hiS[i];
+                            const uint32_t *np = nonS + i + 1;
+                            const uint8_t *hp = hiS + i + 1;
                             uint2 *dst = q.t2_rec + (base2 + e0);
                             uint8_t *dsth = q.t2_hi + (base2 + e0);
-                            // the first four successors unconditionally (positions up to CAPA + 3 lie inside the
-                            // arrays' padding), their loads issued together; longer runs take the loop
-                            uint32_t kj[4], bj[4];
+                            uint32_t nj[4], hj[4];
 #pragma unroll
-                            for (uint32_t t = 0; t < 4; t++) { kj[t] = k32[2 * (i + 1 + t)]; bj[t] = nonS[min(i + 1 + t, (uint32_t)CAPA - 1u)]; }
+                            for (uint32_t t = 0; t < 4; t++) { nj[t] = np[t]; hj[t] = hp[t]; }
 #pragma unroll
                             for (uint32_t t = 0; t < 4; t++)
                                 if (t < c) {
-                                    const uint32_t h = kj[t] & lm;
-                                    dst[t] = make_uint2(ni, (h << nlo) | bj[t]);
-                                    dsth[t] = (uint8_t)(nih | ((h >> (32u - nlo)) << 4));
+                                    dst[t] = make_uint2(ni, nj[t]);
+                                    dsth[t] = (uint8_t)(nih | (hj[t] << 4));
                                 }
                             for (uint32_t t = 4; t < cmax; t++)
                                 if (t < c) {
-                                    const uint32_t h = k32[2 * (i + 1 + t)] & lm;
-                                    dst[t] = make_uint2(ni, (h << nlo) | nonS[i + 1 + t]);
-                                    dsth[t] = (uint8_t)(nih | ((h >> (32u - nlo)) << 4));
+                                    dst[t] = make_uint2(ni, np[t]);
+                                    dsth[t] = (uint8_t)(nih | ((uint32_t)hp[t] << 4));
                                 }
                         } else {
                             const uint32_t ni = nonS[i];
@@ -643,8 +642,14 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                 if (idx < cnt) {
                     const uint64_t k = keyS[idx];
                     if constexpr (WIDE) {
+                        const uint32_t b = nonS[idx];
                         reinterpret_cast<unsigned long long *>(src)[idx] = k;
-                        src_b[idx] = (unsigned short)nonS[idx];
+                        src_b[idx] = (unsigned short)b;
+                        // for the emit: nonce = (low pb key bits) << tile_log | the tile_log bits kept beside the key.
+                        // pb <= 24, so only the LOW key word is needed and everything is 32-bit arithmetic
+                        const uint32_t h = (uint32_t)k & (uint32_t)q.lowmask;
+                        nonS[idx] = (h << q.nlo_bits) | b;
+                        hiS[idx] = (uint8_t)(h >> (32u - q.nlo_bits));
                     } else {
                         src[idx] = make_uint4((uint32_t)k, (uint32_t)(k >> 32), nonS[idx], 0u);
                     }
@@ -1273,7 +1278,7 @@ size_t vx_stage2_smem_bytes(const VxGeom &g)
     const size_t CAPA = g.tile_log == VX_TILE_LOG_BIG ? (size_t)VX_S2B_THREADS * VX_S2B_ITEMS
                                                       : (size_t)VX_S2_THREADS * VX_S2_ITEMS;
     const size_t nbins = (size_t)1 << g.tile_log;
-    return (CAPA + 8) * 8 + CAPA * 4 + (nbins + 32) * 4 + (CAPA + 32) * 4;
+    return (CAPA + 8) * 8 + CAPA * 4 + (nbins + 32) * 4 + (CAPA + 32) * 4 + (g.wide ? CAPA + 16 : 0);
 }
 
 #define VX_S2_KERNEL(WIDE) vx_k_sort_match<VX_S2_THREADS, VX_S2_ITEMS, VX_TILE_LOG, VX_S2_MINB, WIDE>
@@ -1296,10 +1301,14 @@ cudaError_t vx_stage2_configure(void)
     const int small = (int)vx_stage2_smem_bytes(g);
     g.tile_log = VX_TILE_LOG_BIG;
     const int big = (int)vx_stage2_smem_bytes(g);
+    g.wide = 1;                                         // + the emit's byte of high nonce bits per record
+    const int big_wide = (int)vx_stage2_smem_bytes(g);
+    g.tile_log = VX_TILE_LOG;
+    const int small_wide = (int)vx_stage2_smem_bytes(g);
     cudaError_t e = cudaFuncSetAttribute(VX_S2_KERNEL(false), cudaFuncAttributeMaxDynamicSharedMemorySize, small);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, small);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, small_wide);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(false), cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL(true), cudaFuncAttributeMaxDynamicSharedMemorySize, big_wide);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2_KERNEL_WL, cudaFuncAttributeMaxDynamicSharedMemorySize, small);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(VX_S2B_KERNEL_WL, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     return e;
