@@ -272,14 +272,21 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             const uint8_t *hp = hiS + i + 1;
                             uint2 *dst = q.t2_rec + (base2 + e0);
                             uint8_t *dsth = q.t2_hi + (base2 + e0);
+                            // (both pointers pinned in registers: ptxas otherwise rebuilds the byte pointer from the
+                            // index for every store, behind a branch of its own -- 7 instructions per byte)
+                            asm volatile("" : "+l"(dst), "+l"(dsth));
+                            __builtin_assume(__isGlobal(dst));
+                            __builtin_assume(__isGlobal(dsth));
                             uint32_t nj[4], hj[4];
 #pragma unroll
                             for (uint32_t t = 0; t < 4; t++) { nj[t] = np[t]; hj[t] = hp[t]; }
 #pragma unroll
+                            for (uint32_t t = 0; t < 4; t++) hj[t] = nih | (hj[t] << 4);
+#pragma unroll
                             for (uint32_t t = 0; t < 4; t++)
                                 if (t < c) {
                                     dst[t] = make_uint2(ni, nj[t]);
-                                    dsth[t] = (uint8_t)(nih | (hj[t] << 4));
+                                    dsth[t] = (uint8_t)hj[t];
                                 }
                             for (uint32_t t = 4; t < cmax; t++)
                                 if (t < c) {
