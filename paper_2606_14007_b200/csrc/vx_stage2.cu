@@ -297,6 +297,9 @@ vx_k_sort_match(const __grid_constant__ VxS2Params q)
                             const uint32_t ni = nonS[i];
                             const uint32_t *np = nonS + i + 1;
                             uint2 *dst = q.t2_rec + (base2 + e0);
+                            // (pinned in registers: ptxas otherwise rebuilds the pointer from the index for every store)
+                            asm volatile("" : "+l"(dst));
+                            __builtin_assume(__isGlobal(dst));
 #pragma unroll
                             for (uint32_t t = 0; t < 4; t++)
                                 if (t < c) dst[t] = make_uint2(ni, np[t]);
